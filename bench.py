@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the RGF hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (lead decimation A2, sweep A3-A5 over all L slices,
+trace A6) over the headline batch: BASELINE.json configs[2], M=244, L=8000, 512 energies in
+[-1, 1] eV, Anderson disorder +-0.1 eV (seed 5300), complex128, synthetic seeded input.
+Metric: RGF slice-steps/s (slice-step = one (seed, energy, slice) triple).
+
+  value      inputs resident in HBM (energies / T_out are device tensors, ribbon already set)
+  e2e        the same through the C ABI with HOST buffers: rgf_set_device(host onsite) +
+             rgf_transmission(host energies -> host T) inside the timed region
+  roofline   dominant kernel = gj_update_kernel (FP64 DMMA): algorithmic flops per launch divided
+             by its mean CUDA-event duration inside the timed region, against the FP64 tensor
+             ceiling measured live on the same GPU (rgf_fp64_peak_tflops)
+  cpu_baseline  the oracle (oracle/rgf_oracle.c, naive LU, OpenMP over energies) on a bounded sample
+
+--impl reference times the CPU oracle alone (there is no reference implementation to install:
+/root/reference holds only the paper's text).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1107_5300_b200 import inputs  # noqa: E402
+
+METRIC = "rgf_slice_steps_per_s"
+UNIT = "slice-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    # exploration knobs (the driver never passes them; defaults = the headline workload)
+    ap.add_argument("--M", type=int, default=244)
+    ap.add_argument("--L", type=int, default=8000)
+    ap.add_argument("--n-E", type=int, default=512)
+    ap.add_argument("--cohort", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(a, world, rank):
+    """Headline ribbon; with N GPUs the global grid has 512*N energies and rank r takes E[r::N] (weak scaling)."""
+    w = inputs.config2(M=a.M, L=a.L, n_E=a.n_E * world)
+    E = np.ascontiguousarray(w.energies[rank::world])
+    return w, E
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        self.rows, self.proc, self.thread = [], None, None
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + q, "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def update_flops_per_inverse(n, B=32):
+    """Algorithmic real flops of the gj_update launches of one n x n inverse (8 per complex MAC)."""
+    tot, launches = 0, 0
+    for k0 in range(0, n, B):
+        bw = min(B, n - k0)
+        if n > B:
+            tot += 8 * n * (n - bw) * bw
+            launches += 1
+    return tot, launches
+
+
+def cpu_baseline(a, cores_hint=0):
+    """Oracle steady-state sweep rate: (time at L2 slices) - (time at L1 slices), same energies, all cores."""
+    from oracle import rgf_oracle as orc
+    w = inputs.config2(M=a.M, L=max(a.L, 64), n_E=a.n_E)
+    nthr = orc.num_threads()
+    idx = np.linspace(0, w.n_E - 1, nthr).astype(int)
+    E = w.energies[idx]
+    # scale the sample to ~10-30 s: the naive step costs ~ (7/3) M^3 complex MACs
+    per_step = 2.4e-9 * 2.4 * a.M ** 3
+    L2 = int(min(max(8, 12.0 / per_step), 96, w.L))
+    L1 = max(1, L2 // 4)
+    times = []
+    for Lx in (L1, L2):
+        ws = inputs.truncate(w, Lx)
+        t0 = time.perf_counter()
+        orc.transmission_batch(ws.onsite[0], None, ws.t, E, ws.eta, method=orc.LEAD_BLOCK, nthreads=nthr)
+        times.append(time.perf_counter() - t0)
+    dt = max(times[1] - times[0], 1e-9)
+    rate = len(E) * (L2 - L1) / dt
+    return {"value": rate, "unit": UNIT, "cores": nthr, "kind": "oracle",
+            "sample": "%d energies x (%d - %d) slices of the M=%d headline ribbon, lead time cancels in the difference; %.1f s of wall time"
+                      % (len(E), L2, L1, a.M, sum(times))}
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    base = None
+    t_all = []
+    for s in range(a.warmup + a.steps):
+        t0 = time.perf_counter()
+        base = cpu_baseline(a)
+        if s >= a.warmup:
+            t_all.append(time.perf_counter() - t0)
+        if s == 0 and a.warmup + a.steps > 2 and (time.perf_counter() - t0) > 60:
+            break           # keep the whole run within a few minutes
+    val = base["value"]
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": 1e3 * (np.mean(t_all) if t_all else 0.0), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": "configs[2] M=%d L=%d n_E=%d complex128 (bounded sample, see cpu_baseline.sample)" % (a.M, a.L, a.n_E)},
+            "cpu_baseline": base, "gpu_launches": 0,
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    a = parse()
+    if a.impl == "reference":
+        return run_reference(a)
+    import torch
+    from paper_1107_5300_b200 import binding as rgf     # fails loudly if the CUDA library is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    w, E_host = workload(a, world, rank)
+    n_E = len(E_host)
+    onsite = np.ascontiguousarray(w.onsite[0])
+    stream = torch.cuda.current_stream()
+    plan = rgf.rgf_plan_create(local, stream.cuda_stream)
+    if a.cohort:
+        rgf.rgf_set_cohort(plan, a.cohort)
+    peak = rgf.rgf_fp64_peak_tflops(plan)
+    rgf.rgf_set_device(plan, w.M, w.L, onsite, w.t, None)
+    E_dev = torch.from_numpy(E_host).to(dev)
+    T_dev = torch.empty(n_E, dtype=torch.float64, device=dev)
+    rgf.rgf_set_profiling(plan, 1)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step_resident():
+        rgf.rgf_transmission(plan, E_dev, n_E, w.eta, rgf.RGF_C128, T_dev)
+
+    for _ in range(a.warmup):
+        step_resident()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches, ms_upd, n_upd, stats = 0, 0.0, 0, None
+    e0.record()
+    for _ in range(a.steps):
+        step_resident()
+        stats = rgf.rgf_get_stats(plan)
+        launches += stats["launches"]; ms_upd += stats["ms_inverse_update"]; n_upd += stats["launches_inverse_update"]
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    T_first = T_dev.cpu().numpy().copy()
+
+    # ---- e2e: host buffers, set_device + transmission inside the timed region
+    e2e = None
+    if not a.no_e2e:
+        rgf.rgf_set_profiling(plan, 0)
+        E_pin = torch.from_numpy(E_host.copy()).pin_memory()
+        on_pin = torch.from_numpy(onsite.copy()).pin_memory()
+        T_pin = torch.empty(n_E, dtype=torch.float64).pin_memory()
+        e2e_steps = max(1, min(a.steps, 1 if ms / a.steps > 20000 else a.steps))
+        barrier()
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e2.record()
+        for _ in range(e2e_steps):
+            rgf.rgf_set_device(plan, w.M, w.L, on_pin.numpy(), w.t, None)
+            rgf.rgf_transmission(plan, E_pin.numpy(), n_E, w.eta, rgf.RGF_C128, T_pin.numpy())
+        e3.record()
+        barrier()
+        ms_e2e = e2.elapsed_time(e3)
+        assert np.allclose(T_pin.numpy(), T_first, rtol=0, atol=1e-9, equal_nan=True)
+        e2e = (ms_e2e, e2e_steps)
+
+    tmax = torch.tensor([ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max, ms_e2e_max = float(tmax[0]), float(tmax[1])
+    units_step = world * n_E * w.L                        # slice-steps per step over all ranks
+    if rank == 0:
+        value = units_step * a.steps / (ms_max * 1e-3)
+        fl_inv, l_inv = update_flops_per_inverse(w.M)
+        flops_per_launch = fl_inv / max(l_inv, 1) * stats["cohort"]
+        avg_ms = ms_upd / max(n_upd, 1)
+        achieved = flops_per_launch / (avg_ms * 1e-3) * 1e-12 if avg_ms > 0 else 0.0
+        flops_step = n_E * w.L * (8.0 * w.M ** 3 + 8.0 * (w.M / 2) ** 3)      # executed: dense inverse + compact propagator
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[2] armchair ribbon M=%d L=%d n_E=%d per GPU, Anderson +-0.1 eV seed 5300, complex128" % (w.M, w.L, n_E),
+                       "eta": w.eta, "t": w.t, "cohort": stats["cohort"],
+                       "l2_policy": "inputs larger than L2 (%.0f MB of state per step)" % (stats["cohort"] * w.M * w.M * 16 / 1e6)},
+            "energies_per_s": world * n_E * a.steps / (ms_max * 1e-3),
+            "tflops_executed": flops_step * world * a.steps / (ms_max * 1e-3) * 1e-12,
+            "tflops_dense_equivalent": 16.0 * w.M ** 3 * units_step * a.steps / (ms_max * 1e-3) * 1e-12,
+            "phase_ms_last_step": {k: stats[k] for k in ("ms_total", "ms_leads", "ms_sweep", "ms_trace", "ms_inverse_update")},
+            "lead_iterations": stats["lead_iterations"],
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "roofline": {"bound": "tensor", "kernel": "gj_update_kernel<32> (FP64 DMMA.8x8x4)", "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": None,
+                         "peak_source": "measured live: rgf_fp64_peak_tflops (DMMA issue rate, this GPU)",
+                         "launches_timed": n_upd, "share_of_step": ms_upd / ms if ms else None},
+        }
+        if e2e:
+            line["e2e"] = {"value": units_step * e2e[1] / (ms_e2e_max * 1e-3), "unit": UNIT, "steps": e2e[1],
+                           "h2d_bytes_per_step": int(onsite.nbytes + E_host.nbytes), "d2h_bytes_per_step": int(T_first.nbytes)}
+        if not a.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(a)
+        elif world > 1:
+            line["cpu_baseline"] = None
+        print(json.dumps(line))
+    rgf.rgf_destroy(plan)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,138 @@
+/*
+ * rgf.h -- C ABI of the B200 (sm_100a) recursive Green's function library.
+ *
+ * What the library computes: the Landauer transmission T(E) of an armchair graphene
+ * nanoribbon (one p_z orbital per atom, nearest-neighbour hopping t) between two clean
+ * semi-infinite leads of the same width, by the recursive Green's function sweep of
+ *   S. Ihnatsenka, Comput. Phys. Commun. 183 (2012) 543 (arXiv:1107.5300):
+ *     PAPER.md:33-37  Eq. 1   G = (E - H)^-1
+ *     PAPER.md:37-41  Eq. 2   conductance = (2e^2/h) Tr[Gamma_L G^a Gamma_R G^r]
+ *     PAPER.md:45-53  Eq. 4-5 slice recursion  G_jj, G_1j  (one solver call + GEMMs per slice)
+ *     PAPER.md:53,58  lead self-energies added at the first and the last slice
+ * in the direct form of BASELINE.json:north_star, with z = E + i*eta:
+ *     G_ii   = (z - H_i - V G_{i-1,i-1} V)^-1            (complex M x M inverse)
+ *     G_{i,0} = G_ii V G_{i-1,0}                           (complex GEMM)
+ *     Sigma_L/R from Sancho-Rubio decimation of the clean two-slice lead cell
+ *     T(E) = Re Tr[Gamma_L G_{L-1,0}^dagger Gamma_R G_{L-1,0}],  Gamma = i(Sigma - Sigma^dagger)
+ *
+ * Geometry (BASELINE.json:configs[0]): M atoms per slice (matrix size),
+ * L slices, 0-based slice i and atom j.  H_i = diag(onsite[i][:]) + t on the first sub/super
+ * diagonal; V_{i,i+1} = t*diag(m_i), m_i[j] = 1 iff (i+j) even.  A vacancy zeroes every
+ * hopping that touches the site (it stays an isolated level at its on-site energy).
+ *
+ * Every step runs in CUDA kernels of this library; there is no CPU fallback.  All entry
+ * points return RGF_OK (0) or a negative error code, never throw, never abort.
+ *
+ * Pointers: unless stated otherwise an array argument may be a HOST pointer or a CUDA DEVICE
+ * pointer on the plan's device (the library asks cudaPointerGetAttributes); the caller owns
+ * every array, and the library never keeps a caller pointer after the call returns.
+ */
+#ifndef RGF_H
+#define RGF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rgf_plan rgf_plan;          /* opaque; created by rgf_plan_create, freed by rgf_destroy */
+
+enum { RGF_C128 = 0, RGF_C64 = 1 };        /* precision of the sweep (assembly, inverse, propagator) */
+
+enum {
+    RGF_OK = 0,
+    RGF_EINVAL = -1,       /* bad argument (NULL, M < 2, L < 1, n_E < 1, eta <= 0, non-finite, ...) */
+    RGF_ECUDA = -2,        /* a CUDA call failed; see rgf_last_error                              */
+    RGF_ENOMEM = -3,       /* host or device allocation failed                                    */
+    RGF_ENOCONV = -4,      /* lead decimation hit the iteration cap for at least one energy       */
+    RGF_ESINGULAR = -5,    /* zero or non-finite pivot in at least one inverse                    */
+    RGF_ESTATE = -6,       /* rgf_transmission before rgf_set_device                              */
+    RGF_EUNSUPPORTED = -7  /* precision / size not built in this version                          */
+};
+
+/* Create an empty plan bound to CUDA device `cuda_device`.  `cuda_stream` is a cudaStream_t
+ * (e.g. torch.cuda.current_stream().cuda_stream) on which all work is enqueued, or NULL for a
+ * stream owned by the plan.  *out receives the plan. */
+int rgf_plan_create(rgf_plan **out, int cuda_device, void *cuda_stream);
+
+/* Describe one ribbon (region of length L between two leads of the same width).
+ *   onsite  [L][M] row-major doubles, eV
+ *   t       hopping, eV (e.g. -2.7)
+ *   vacancy [L][M] bytes, 1 = vacant site, or NULL for none
+ * The arrays are copied to the device; the caller may free them on return.  A second call
+ * replaces the device (buffers are reused when M and L are unchanged). */
+int rgf_set_device(rgf_plan *p, int M, int L, const double *onsite, double t, const uint8_t *vacancy);
+
+/* Batched variant: n_dev ribbons (disorder seeds) of the same M, L, t
+ * (BASELINE.json:configs[1] "4 disorder seeds batched").  onsite [n_dev][L][M],
+ * vacancy [n_dev][L][M] or NULL.  rgf_transmission then writes T_out[n_dev][n_E]. */
+int rgf_set_device_batch(rgf_plan *p, int n_dev, int M, int L, const double *onsite, double t,
+                         const uint8_t *vacancy);
+
+/* T(E) for n_E energies (eV), broadening eta > 0 (eV), sweep precision RGF_C128 / RGF_C64.
+ * T_out[n_dev][n_E] doubles (n_dev = 1 after rgf_set_device).  Synchronous: T_out is valid on
+ * return.  Runs leads (A2), the sweep (A3-A5) and the trace (A6) on the GPU.  On a per-energy
+ * failure that entry of T_out is NaN, the other energies are still computed, and the code
+ * (RGF_ENOCONV / RGF_ESINGULAR) is returned. */
+int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, int precision,
+                     double *T_out);
+
+/* Free the plan and everything it owns.  NULL is accepted. */
+int rgf_destroy(rgf_plan *p);
+
+/* Message of the last error on this plan (plan-owned, valid until the next call), or a static
+ * string if p is NULL. */
+const char *rgf_last_error(const rgf_plan *p);
+
+/* ---- counters of the last rgf_transmission call -------------------------------------- */
+typedef struct rgf_stats {
+    double ms_total;            /* CUDA-event time of the whole call on the plan's stream       */
+    double ms_leads;            /* lead decimation                                               */
+    double ms_sweep;            /* assembly + inverse + propagator over all slices              */
+    double ms_trace;            /* Gamma trace + download                                        */
+    double ms_inverse_update;   /* summed CUDA-event time of the Gauss-Jordan update kernel      */
+    long long launches;         /* kernels launched by the call                                  */
+    long long launches_inverse_update; /* gj_update launches of the sweep (the ones timed)            */
+    long long launches_leads;   /* kernels launched by the lead decimation                       */
+    int lead_iterations;        /* decimation iterations run (max over energies)                 */
+    int cohort;                 /* matrices per launch                                           */
+} rgf_stats;
+int rgf_get_stats(const rgf_plan *p, rgf_stats *out);
+
+/* Timing detail: 0 = whole-call events only (default), 1 = also bracket every inverse-update
+ * launch with events (adds a little launch overhead; used by bench.py for the roofline line). */
+int rgf_set_profiling(rgf_plan *p, int level);
+
+/* Matrices per kernel launch in the sweep (0 = library default = the whole batch).  The sweep runs
+ * cohort after cohort over all slices; a cohort whose state fits the 126 MB L2 keeps it there. */
+int rgf_set_cohort(rgf_plan *p, int cohort);
+
+/* Measures the FP64 tensor-pipe ceiling of the plan's GPU (independent DMMA.8x8x4 chains on every
+ * warp, 2 CTAs x 16 warps per SM) and writes it in TFLOP/s; the roofline denominator of bench.py. */
+int rgf_fp64_peak_tflops(rgf_plan *p, double *tflops_out);
+
+/* ---- sub-steps, exported so that each row of the hot path can be checked on its own ---- */
+
+/* A4 alone: inverse of `batch` complex n x n matrices (interleaved re,im doubles, row-major,
+ * matrix b at A + b*n*n*2 doubles) by the library's blocked Gauss-Jordan with partial
+ * pivoting.  A and Ainv may be host or device pointers; Ainv may equal A. */
+int rgf_inverse_batched(rgf_plan *p, int n, int batch, const double *A, double *Ainv);
+
+/* A2 alone: lead self-energies Sigma_L (side = -1) or Sigma_R (side = +1) of device `dev`
+ * for n_E energies: Sigma_out[n_E][M][M] interleaved complex.  iterations_out (host int, may be
+ * NULL) receives the number of decimation iterations run. */
+int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int side,
+                         double *Sigma_out, int *iterations_out);
+
+/* A3-A5 alone: state after the first `nslices` slices (1..L) of the sweep on device `dev`:
+ * g_out[n_E][M][M] = G_ii and P_out[n_E][M][M] = G_{i,0}, i = nslices-1 (interleaved complex).
+ * The library propagates only the rows/columns of G_{i,0} that the rest of the path consumes
+ * (rows with m_i = 1, columns with m_{-1} = 1); every other entry of P_out is written as NaN. */
+int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int precision,
+                    int nslices, double *g_out, double *P_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RGF_H */

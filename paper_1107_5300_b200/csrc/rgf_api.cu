@@ -1,0 +1,772 @@
+// rgf_api.cu -- C ABI (include/rgf.h) and host orchestration of the RGF sweep on one B200.
+//
+// Call stack of rgf_transmission:
+//   leads   : Sancho-Rubio decimation, batched over energies          (A2)  run_leads()
+//   sweep   : for each slice i: assemble A_i (A1+A3) -> blocked Gauss-Jordan inverse (A4)
+//             -> compact propagator GEMM (A5), batched over (device, energy)   run_sweep()
+//   trace   : Gamma_R P, P^dagger (.), masked Gamma_L reduction             (A6)  run_trace()
+// PyTorch is not involved: plain CUDA runtime, one stream, no CPU fallback anywhere.
+#include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "../../include/rgf.h"
+#include "gj_inverse.cuh"
+#include "rgf_common.cuh"
+#include "sweep_kernels.cuh"
+#include "zgemm.cuh"
+
+using namespace rgf;
+
+namespace {
+
+struct Buf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+}  // namespace
+
+struct rgf_plan {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    bool has_device = false;
+    int M = 0, L = 0, n_dev = 0, nh = 0;
+    double t = 0.0;
+    Buf onsite, bond, hop, bondc;                 // device description
+    Buf E, T, status, lead_flags, counters;       // per call
+    Buf G, Nb, Rb, orig, Pa, Pb;                  // sweep workspace (cohort-sized)
+    Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
+    Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_T4, l_W;   // decimation workspace
+    Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
+    int cohort_override = 0;
+    int profiling = 0;
+    bool in_sweep = false;                        // update-kernel events are taken for the sweep's inverses only
+    rgf_stats stats;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
+    size_t upd_used = 0;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    char err[512];
+    bool attrs_set = false;
+};
+
+namespace {
+
+const char *kNoPlan = "rgf: NULL plan";
+
+int fail(rgf_plan *p, int code, const char *fmt, ...)
+{
+    if (p) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(p->err, sizeof(p->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CUDA_TRY(p, call)                                                                              \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail((p), e_ == cudaErrorMemoryAllocation ? RGF_ENOMEM : RGF_ECUDA, "%s failed: %s (%s:%d)", #call, \
+                        cudaGetErrorString(e_), __FILE__, __LINE__);                                   \
+    } while (0)
+
+int ensure(rgf_plan *p, Buf &b, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    if (b.cap >= bytes) return RGF_OK;
+    if (b.p) { CUDA_TRY(p, cudaFree(b.p)); b.p = nullptr; b.cap = 0; }
+    CUDA_TRY(p, cudaMalloc(&b.p, bytes));
+    b.cap = bytes;
+    return RGF_OK;
+}
+
+void release(Buf &b)
+{
+    if (b.p) cudaFree(b.p);
+    b.p = nullptr;
+    b.cap = 0;
+}
+
+template <typename T> T *ptr(const Buf &b) { return reinterpret_cast<T *>(b.p); }
+
+int set_kernel_attrs(rgf_plan *p)
+{
+    if (p->attrs_set) return RGF_OK;
+    CUDA_TRY(p, cudaFuncSetAttribute(zgemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ZG_SMEM));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<32>()));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<16>()));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<8>()));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_panel2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj_panel2_smem(256)));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
+    p->attrs_set = true;
+    return RGF_OK;
+}
+
+inline int panel_width(int n) { return n <= 256 ? 32 : (n <= 512 ? 16 : 8); }
+
+int launch_zgemm(rgf_plan *p, const ZgemmArgs &a, int batch)
+{
+    if (a.Mr <= 0 || a.Nc <= 0 || batch <= 0) return RGF_OK;
+    dim3 grid((a.Nc + ZG_BN - 1) / ZG_BN, (a.Mr + ZG_BM - 1) / ZG_BM, batch);
+    zgemm_kernel<<<grid, ZG_THREADS, ZG_SMEM, p->stream>>>(a);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    return RGF_OK;
+}
+
+template <int B, int NT>
+void launch_panel(rgf_plan *p, cplx *G, int n, int batch, int k0, cplx *Nb, cplx *Rb, int *orig, int *status)
+{
+    gj_panel_kernel<B, NT><<<batch, NT, gj_panel_smem<B>(n), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+}
+
+template <int B>
+int inverse_impl(rgf_plan *p, cplx *G, int n, int batch, int *status)
+{
+    cplx *Nb = ptr<cplx>(p->Nb), *Rb = ptr<cplx>(p->Rb);
+    int *orig = ptr<int>(p->orig);
+    int total = n * batch;
+    gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, p->stream>>>(orig, n, total);
+    p->stats.launches++;
+    for (int k0 = 0; k0 < n; k0 += B) {
+        if (B == 32) {
+            gj_panel2_kernel<<<batch, P2_NT, gj_panel2_smem(n), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+        } else if (B == 16) {
+            launch_panel<16, 512>(p, G, n, batch, k0, Nb, Rb, orig, status);
+        } else {
+            launch_panel<8, 1024>(p, G, n, batch, k0, Nb, Rb, orig, status);
+        }
+        p->stats.launches++;
+        CUDA_TRY(p, cudaGetLastError());
+        if (n > B) {
+            dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
+            bool timed = p->profiling > 0 && p->in_sweep;
+            cudaEvent_t e0 = nullptr, e1 = nullptr;
+            if (timed) {
+                if (p->upd_used == p->upd_events.size()) {
+                    if (p->upd_events.size() >= 2048) {
+                        // drain: accumulate and reuse
+                        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+                        for (size_t q = 0; q < p->upd_used; q++) {
+                            float ms = 0.f;
+                            cudaEventElapsedTime(&ms, p->upd_events[q].first, p->upd_events[q].second);
+                            p->stats.ms_inverse_update += ms;
+                        }
+                        p->upd_used = 0;
+                    } else {
+                        cudaEvent_t a, b;
+                        CUDA_TRY(p, cudaEventCreate(&a));
+                        CUDA_TRY(p, cudaEventCreate(&b));
+                        p->upd_events.push_back(std::make_pair(a, b));
+                    }
+                }
+                e0 = p->upd_events[p->upd_used].first;
+                e1 = p->upd_events[p->upd_used].second;
+                p->upd_used++;
+                CUDA_TRY(p, cudaEventRecord(e0, p->stream));
+            }
+            gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb);
+            if (timed) CUDA_TRY(p, cudaEventRecord(e1, p->stream));
+            p->stats.launches++;
+            if (p->in_sweep) p->stats.launches_inverse_update++;
+            CUDA_TRY(p, cudaGetLastError());
+        }
+    }
+    int nw = n > 512 ? 4 : 8;
+    dim3 grid((n + nw - 1) / nw, batch);
+    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), p->stream>>>(G, (long long)n * n, n, orig);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    return RGF_OK;
+}
+
+// workspace for inverting `batch` n x n matrices
+int ensure_inverse_ws(rgf_plan *p, int n, int batch)
+{
+    int B = panel_width(n), rc;
+    if ((rc = ensure(p, p->Nb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
+    if ((rc = ensure(p, p->Rb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
+    if ((rc = ensure(p, p->orig, sizeof(int) * (size_t)n * batch))) return rc;
+    return RGF_OK;
+}
+
+// in-place inverse of `batch` matrices stored at G (stride n*n); status[b] set to 1 on a bad pivot
+int run_inverse(rgf_plan *p, cplx *G, int n, int batch, int *status)
+{
+    if (n > 1024) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 1024 is not supported in this version", n);
+    int B = panel_width(n);
+    if (B == 32) return inverse_impl<32>(p, G, n, batch, status);
+    if (B == 16) return inverse_impl<16>(p, G, n, batch, status);
+    return inverse_impl<8>(p, G, n, batch, status);
+}
+
+void drain_update_events(rgf_plan *p)
+{
+    for (size_t q = 0; q < p->upd_used; q++) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p->upd_events[q].first, p->upd_events[q].second) == cudaSuccess)
+            p->stats.ms_inverse_update += ms;
+    }
+    p->upd_used = 0;
+}
+
+}  // namespace
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// A2. Lead surface Green's functions g_L (slice -1) and g_R (slice L) for n_E energies.
+// Sancho-Rubio decimation on the clean two-slice lead cell (BASELINE.json:north_star item 4):
+//   g = (z - eps)^-1; eps_s += (towards the bulk); eps += a g b + b g a; a <- a g a; b <- b g b
+// on the 2M x 2M cell until max|a|, max|b| < 1e-14 eV for every energy (cap 64 iterations).
+// side -1: V_a = t diag(m_{-2}), V_b = t diag(m_{-1});  side +1: V_a = t diag(m_L), V_b = t diag(m_{L+1}).
+// ------------------------------------------------------------------------------------------
+constexpr double kLeadTol = 1e-14;
+constexpr int kLeadMaxIt = 64;
+
+// C (M x M, ld = M) = A (M x M, ld lda) * B (M x M, ld ldb), batched over n_E
+int lead_gemm(rgf_plan *p, const cplx *A, int lda, long long a_batch, const cplx *B, int ldb, long long b_batch, cplx *C, int n_E)
+{
+    const int M = p->M;
+    ZgemmArgs a;
+    memset(&a, 0, sizeof(a));
+    a.A = A; a.a_batch = a_batch; a.a_rs = lda; a.a_cs = 1; a.kmask_div = 1;
+    a.B = B; a.b_batch = b_batch; a.ldb = ldb;
+    a.C = C; a.c_batch = (long long)M * M; a.ldc = M;
+    a.Mr = a.Nc = a.K = M;
+    a.alpha = cmake(1.0, 0.0);
+    return launch_zgemm(p, a, n_E);
+}
+
+int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cplx *g_out, int *iters_out, int *n_open_out)
+{
+    const int M = p->M, N = 2 * M;
+    if (N > 1024) return fail(p, RGF_EUNSUPPORTED, "lead decimation needs a %d x %d inverse; M > 512 is not supported in this version", N, N);
+    const long long MM = (long long)M * M, NN = (long long)N * N;
+    int rc;
+    if ((rc = ensure(p, p->l_eps, sizeof(cplx) * NN * n_E))) return rc;
+    if ((rc = ensure(p, p->l_eps_s, sizeof(cplx) * NN * n_E))) return rc;
+    if ((rc = ensure(p, p->l_W, sizeof(cplx) * NN * n_E))) return rc;
+    Buf *small[] = {&p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4};
+    for (Buf *b : small) if ((rc = ensure(p, *b, sizeof(cplx) * MM * n_E))) return rc;
+    if ((rc = ensure_inverse_ws(p, N, n_E))) return rc;
+    if ((rc = ensure(p, p->lead_flags, sizeof(int) * (size_t)(n_E + 4)))) return rc;
+    cplx *eps = ptr<cplx>(p->l_eps), *eps_s = ptr<cplx>(p->l_eps_s), *g = ptr<cplx>(p->l_W);
+    cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta);
+    cplx *T1 = ptr<cplx>(p->l_T1), *X = ptr<cplx>(p->l_T2), *Y = ptr<cplx>(p->l_T3), *T3 = ptr<cplx>(p->l_T4);
+    int *flags = ptr<int>(p->lead_flags), *n_open = flags + n_E;
+    int *status = ptr<int>(p->status);      // a bad pivot in the lead marks batch items [0, n_E): device 0 of each energy
+    const double *E = ptr<double>(p->E);
+    dim3 gN((unsigned)std::min<long long>((NN + 255) / 256, 2048), n_E), gM((unsigned)std::min<long long>((MM + 255) / 256, 1024), n_E);
+    const cplx *g11 = g, *g12 = g + M, *g21 = g + (long long)M * N, *g22 = g + (long long)M * N + M;
+
+    lead_cell_init_kernel<<<gN, 256, 0, p->stream>>>(eps, eps_s, a, b, M, p->t, pa, pb);
+    p->stats.launches++;
+    int it = 0, open = n_E;
+    for (it = 0; it < kLeadMaxIt; it++) {
+        CUDA_TRY(p, cudaMemsetAsync(n_open, 0, sizeof(int), p->stream));
+        lead_converged_kernel<<<n_E, 256, 0, p->stream>>>(a, b, M, kLeadTol, flags, n_open);
+        p->stats.launches++;
+        CUDA_TRY(p, cudaMemcpyAsync(&open, n_open, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
+        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        if (open == 0) break;
+        lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(g, eps, N, E, eta);
+        p->stats.launches++;
+        if ((rc = run_inverse(p, g, N, n_E, status))) return rc;
+        if ((rc = lead_gemm(p, a, M, MM, g11, N, NN, T1, n_E))) return rc;      // a g11
+        if ((rc = lead_gemm(p, T1, M, MM, b, M, MM, X, n_E))) return rc;        // X = a g11 b   -> [2,2]
+        if ((rc = lead_gemm(p, b, M, MM, g22, N, NN, T3, n_E))) return rc;      // b g22
+        if ((rc = lead_gemm(p, T3, M, MM, a, M, MM, Y, n_E))) return rc;        // Y = b g22 a   -> [1,1]
+        lead_cell_accumulate_kernel<<<gM, 256, 0, p->stream>>>(eps, eps_s, X, Y, M, side);
+        p->stats.launches++;
+        if ((rc = lead_gemm(p, a, M, MM, g12, N, NN, T1, n_E))) return rc;      // a g12
+        if ((rc = lead_gemm(p, T1, M, MM, a, M, MM, X, n_E))) return rc;        // a g12 a
+        if ((rc = lead_gemm(p, b, M, MM, g21, N, NN, T3, n_E))) return rc;      // b g21
+        if ((rc = lead_gemm(p, T3, M, MM, b, M, MM, Y, n_E))) return rc;        // b g21 b
+        std::swap(a, X);
+        std::swap(b, Y);
+    }
+    lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(g, eps_s, N, E, eta);
+    p->stats.launches++;
+    if ((rc = run_inverse(p, g, N, n_E, status))) return rc;
+    lead_extract_kernel<<<gM, 256, 0, p->stream>>>(g, g_out, M, side);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    if (iters_out) *iters_out = it;
+    if (n_open_out) *n_open_out = open;
+    return RGF_OK;
+}
+
+// both leads; for even L the two cells have the same bond parities and g_R = g_L exactly
+int run_leads(rgf_plan *p, int n_E, double eta, int *n_open_out)
+{
+    const int M = p->M, L = p->L;
+    int rc, itL = 0, itR = 0, openL = 0, openR = 0;
+    const size_t MMb = sizeof(cplx) * (size_t)M * M * n_E;
+    if ((rc = ensure(p, p->gL, MMb))) return rc;
+    if ((rc = run_lead_side(p, n_E, eta, -1, -2, -1, ptr<cplx>(p->gL), &itL, &openL))) return rc;
+    if ((L & 1) == 0) {
+        itR = itL; openR = 0;      // g_R aliases g_L (see pR() below)
+    } else {
+        if ((rc = ensure(p, p->gR, MMb))) return rc;
+        if ((rc = run_lead_side(p, n_E, eta, +1, L, L + 1, ptr<cplx>(p->gR), &itR, &openR))) return rc;
+    }
+    p->stats.lead_iterations = std::max(itL, itR);
+    if (n_open_out) *n_open_out = openL + openR;
+    return RGF_OK;
+}
+
+inline const cplx *lead_gR(const rgf_plan *p) { return (p->L & 1) == 0 ? ptr<cplx>(p->gL) : ptr<cplx>(p->gR); }
+
+int choose_cohort(const rgf_plan *p, int batch)
+{
+    if (p->cohort_override > 0) return std::min(p->cohort_override, batch);
+    return batch;
+}
+
+int ensure_sweep_ws(rgf_plan *p, int cohort)
+{
+    int rc;
+    const int M = p->M, nh = p->nh;
+    if ((rc = ensure(p, p->G, sizeof(cplx) * (size_t)M * M * cohort))) return rc;
+    if ((rc = ensure(p, p->Pa, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
+    if ((rc = ensure(p, p->Pb, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
+    return ensure_inverse_ws(p, M, cohort);
+}
+
+// A3-A5 for the cohort [bz0, bz0+nb): slices 0..nslices-1.  On return G holds g_{nslices-1} and
+// *Pcur the compact propagator.
+int run_sweep_cohort(rgf_plan *p, int n_E, double eta, int bz0, int nb, int nslices, cplx **Pcur_out)
+{
+    const int M = p->M, L = p->L, nh = p->nh;
+    int rc;
+    cplx *G = ptr<cplx>(p->G), *Pcur = ptr<cplx>(p->Pa), *Pnext = ptr<cplx>(p->Pb);
+    int *status = ptr<int>(p->status) + bz0;
+    const double *E = ptr<double>(p->E);
+    dim3 ag((unsigned)std::min<long long>(((long long)M * M + 255) / 256, 2048), nb);
+    for (int i = 0; i < nslices; i++) {
+        assemble_kernel<<<ag, 256, 0, p->stream>>>(G, M, L, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite),
+                                                  ptr<uint8_t>(p->bond), ptr<uint8_t>(p->hop), ptr<cplx>(p->gL), lead_gR(p));
+        p->stats.launches++;
+        if ((rc = run_inverse(p, G, M, nb, status))) return rc;
+        if (i == 0) {
+            dim3 pg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
+            propagator_start_kernel<<<pg, 256, 0, p->stream>>>(G, Pcur, M, nh);
+            p->stats.launches++;
+        } else {
+            // P_i[S_i, :] = t * g_i[S_i, S_{i-1}] diag(m'_{i-1}) P_{i-1}[S_{i-1}, :]   (Eq. 5)
+            const int pi = i & 1, pp = (i - 1) & 1;
+            ZgemmArgs a;
+            memset(&a, 0, sizeof(a));
+            a.A = G + (long long)pi * M + pp; a.a_batch = (long long)M * M; a.a_rs = 2LL * M; a.a_cs = 2;
+            a.kmask = ptr<uint8_t>(p->bondc) + (long long)i * nh;                              // m'_{i-1} compact
+            a.kmask_batch = (long long)(L + 1) * nh; a.kmask_div = n_E; a.kmask_b0 = bz0;
+            a.B = Pcur; a.b_batch = (long long)nh * nh; a.ldb = nh;
+            a.C = Pnext; a.c_batch = (long long)nh * nh; a.ldc = nh;
+            a.Mr = (M - pi + 1) / 2; a.K = (M - pp + 1) / 2; a.Nc = M / 2;
+            a.alpha = cmake(p->t, 0.0);
+            if ((rc = launch_zgemm(p, a, nb))) return rc;
+            std::swap(Pcur, Pnext);
+        }
+    }
+    CUDA_TRY(p, cudaGetLastError());
+    *Pcur_out = Pcur;
+    return RGF_OK;
+}
+
+// A6 for the cohort: T = Re Tr[Gamma_L P^dagger Gamma_R P]  (Eq. 2)
+int run_trace_cohort(rgf_plan *p, int n_E, int bz0, int nb, cplx *Pcur)
+{
+    const int M = p->M, L = p->L, nh = p->nh;
+    int rc;
+    cplx *scratch = ptr<cplx>(p->G);                   // g_{L-1} is no longer needed
+    cplx *Gam = scratch, *Y = scratch + (size_t)nh * nh * nb;
+    cplx *X = (Pcur == ptr<cplx>(p->Pa)) ? ptr<cplx>(p->Pb) : ptr<cplx>(p->Pa);
+    const int pR = (L - 1) & 1, nr = (M - pR + 1) / 2, nc = M / 2;
+    dim3 gg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
+    gamma_right_kernel<<<gg, 256, 0, p->stream>>>(Gam, lead_gR(p), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t);
+    p->stats.launches++;
+    ZgemmArgs a;
+    memset(&a, 0, sizeof(a));                            // X = Gamma_R P
+    a.A = Gam; a.a_batch = (long long)nh * nh; a.a_rs = nh; a.a_cs = 1; a.kmask_div = 1;
+    a.B = Pcur; a.b_batch = (long long)nh * nh; a.ldb = nh;
+    a.C = X; a.c_batch = (long long)nh * nh; a.ldc = nh;
+    a.Mr = nr; a.K = nr; a.Nc = nc; a.alpha = cmake(1.0, 0.0);
+    if ((rc = launch_zgemm(p, a, nb))) return rc;
+    memset(&a, 0, sizeof(a));                            // Y = P^dagger X
+    a.A = Pcur; a.a_batch = (long long)nh * nh; a.a_rs = 1; a.a_cs = nh; a.conjA = 1; a.kmask_div = 1;
+    a.B = X; a.b_batch = (long long)nh * nh; a.ldb = nh;
+    a.C = Y; a.c_batch = (long long)nh * nh; a.ldc = nh;
+    a.Mr = nc; a.K = nr; a.Nc = nc; a.alpha = cmake(1.0, 0.0);
+    if ((rc = launch_zgemm(p, a, nb))) return rc;
+    trace_kernel<<<nb, 256, 0, p->stream>>>(Y, ptr<cplx>(p->gL), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t, ptr<double>(p->T));
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    return RGF_OK;
+}
+
+int upload_energies(rgf_plan *p, const double *energies, int n_E, double eta)
+{
+    if (!energies || n_E < 1) return fail(p, RGF_EINVAL, "energies NULL or n_E < 1");
+    if (!(eta > 0.0) || !std::isfinite(eta)) return fail(p, RGF_EINVAL, "eta must be finite and > 0");
+    int rc;
+    if ((rc = ensure(p, p->E, sizeof(double) * (size_t)n_E))) return rc;
+    CUDA_TRY(p, cudaMemcpyAsync(p->E.p, energies, sizeof(double) * (size_t)n_E, cudaMemcpyDefault, p->stream));
+    return RGF_OK;
+}
+
+int begin_call(rgf_plan *p)
+{
+    if (!p) return RGF_EINVAL;
+    p->err[0] = 0;
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    return set_kernel_attrs(p);
+}
+
+}  // namespace
+
+// ==========================================================================================
+// Exported C ABI
+// ==========================================================================================
+extern "C" {
+
+int rgf_plan_create(rgf_plan **out, int cuda_device, void *cuda_stream)
+{
+    if (!out) return RGF_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return RGF_ECUDA;
+    rgf_plan *p = new (std::nothrow) rgf_plan();
+    if (!p) return RGF_ENOMEM;
+    p->err[0] = 0;
+    memset(&p->stats, 0, sizeof(p->stats));
+    p->device = cuda_device;
+    if (cudaSetDevice(cuda_device) != cudaSuccess) { delete p; return RGF_ECUDA; }
+    if (cuda_stream) {
+        p->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    } else {
+        if (cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking) != cudaSuccess) { delete p; return RGF_ECUDA; }
+        p->own_stream = true;
+    }
+    for (int i = 0; i < 5; i++)
+        if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { delete p; return RGF_ECUDA; }
+    *out = p;
+    return RGF_OK;
+}
+
+int rgf_set_device_batch(rgf_plan *p, int n_dev, int M, int L, const double *onsite, double t, const uint8_t *vacancy)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (n_dev < 1 || M < 2 || L < 1 || !onsite || !std::isfinite(t))
+        return fail(p, RGF_EINVAL, "rgf_set_device: need n_dev >= 1, M >= 2, L >= 1, onsite != NULL, finite t");
+    if (M > 1024) return fail(p, RGF_EUNSUPPORTED, "M = %d > 1024 is not supported in this version", M);
+    const size_t nsite = (size_t)n_dev * L * M;
+    // the masks are derived on the host (O(L M) bytes, once per device): bring the inputs here first
+    std::vector<double> h_on(nsite);
+    std::vector<uint8_t> h_vac(nsite, 0);
+    CUDA_TRY(p, cudaMemcpy(h_on.data(), onsite, sizeof(double) * nsite, cudaMemcpyDefault));
+    if (vacancy) CUDA_TRY(p, cudaMemcpy(h_vac.data(), vacancy, nsite, cudaMemcpyDefault));
+    for (size_t k = 0; k < nsite; k++)
+        if (!std::isfinite(h_on[k])) return fail(p, RGF_EINVAL, "onsite[%zu] is not finite", k);
+    const int nh = (M + 1) / 2;
+    std::vector<uint8_t> h_bond((size_t)n_dev * (L + 1) * M), h_hop(nsite), h_bondc((size_t)n_dev * (L + 1) * nh, 0);
+    for (int d = 0; d < n_dev; d++) {
+        const uint8_t *vac = h_vac.data() + (size_t)d * L * M;
+        auto isvac = [&](int i, int j) { return (i >= 0 && i < L) ? vac[(size_t)i * M + j] != 0 : false; };
+        for (int i = -1; i < L; i++) {
+            uint8_t *bm = h_bond.data() + ((size_t)d * (L + 1) + (i + 1)) * M;
+            uint8_t *bc = h_bondc.data() + ((size_t)d * (L + 1) + (i + 1)) * nh;
+            for (int j = 0; j < M; j++) {
+                bm[j] = (mask_bit(i, j) && !isvac(i, j) && !isvac(i + 1, j)) ? 1 : 0;
+                if (mask_bit(i, j)) bc[j >> 1] = bm[j];       // j = 2k + (i & 1)
+            }
+        }
+        for (int i = 0; i < L; i++)
+            for (int j = 0; j < M; j++)
+                h_hop[((size_t)d * L + i) * M + j] = (j + 1 < M && !isvac(i, j) && !isvac(i, j + 1)) ? 1 : 0;
+    }
+    if ((rc = ensure(p, p->onsite, sizeof(double) * nsite))) return rc;
+    if ((rc = ensure(p, p->bond, h_bond.size()))) return rc;
+    if ((rc = ensure(p, p->hop, h_hop.size()))) return rc;
+    if ((rc = ensure(p, p->bondc, h_bondc.size()))) return rc;
+    CUDA_TRY(p, cudaMemcpy(p->onsite.p, h_on.data(), sizeof(double) * nsite, cudaMemcpyHostToDevice));
+    CUDA_TRY(p, cudaMemcpy(p->bond.p, h_bond.data(), h_bond.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(p, cudaMemcpy(p->hop.p, h_hop.data(), h_hop.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(p, cudaMemcpy(p->bondc.p, h_bondc.data(), h_bondc.size(), cudaMemcpyHostToDevice));
+    p->M = M; p->L = L; p->n_dev = n_dev; p->nh = nh; p->t = t;
+    p->has_device = true;
+    return RGF_OK;
+}
+
+int rgf_set_device(rgf_plan *p, int M, int L, const double *onsite, double t, const uint8_t *vacancy)
+{
+    return rgf_set_device_batch(p, 1, M, L, onsite, t, vacancy);
+}
+
+static int check_energies_finite(rgf_plan *p, int n_E)
+{
+    std::vector<double> h(n_E);
+    CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->E.p, sizeof(double) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    for (int k = 0; k < n_E; k++)
+        if (!std::isfinite(h[k])) return fail(p, RGF_EINVAL, "energies[%d] is not finite", k);
+    return RGF_OK;
+}
+
+int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, int precision, double *T_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_transmission before rgf_set_device");
+    if (!T_out) return fail(p, RGF_EINVAL, "T_out is NULL");
+    if (precision != RGF_C128) {
+        if (precision == RGF_C64) return fail(p, RGF_EUNSUPPORTED, "complex64 sweep is not built in this version");
+        return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
+    }
+    memset(&p->stats, 0, sizeof(p->stats));
+    p->upd_used = 0;
+    CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
+    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
+    if ((rc = check_energies_finite(p, n_E))) return rc;
+    const int batch = p->n_dev * n_E;
+    if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
+    if ((rc = ensure(p, p->T, sizeof(double) * (size_t)batch))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    int lead_open = 0;
+    nvtxRangePushA("rgf_leads");
+    rc = run_leads(p, n_E, eta, &lead_open);
+    nvtxRangePop();
+    if (rc) return rc;
+    p->stats.launches_leads = p->stats.launches;
+    CUDA_TRY(p, cudaEventRecord(p->ev[1], p->stream));
+    const int cohort = choose_cohort(p, batch);
+    p->stats.cohort = cohort;
+    if ((rc = ensure_sweep_ws(p, cohort))) return rc;
+    float ms_trace = 0.f;
+    for (int bz0 = 0; bz0 < batch; bz0 += cohort) {
+        const int nb = std::min(cohort, batch - bz0);
+        cplx *Pcur = nullptr;
+        nvtxRangePushA("rgf_sweep");
+        p->in_sweep = true;
+        rc = run_sweep_cohort(p, n_E, eta, bz0, nb, p->L, &Pcur);
+        p->in_sweep = false;
+        nvtxRangePop();
+        if (rc) return rc;
+        nvtxRangePushA("rgf_trace");
+        rc = run_trace_cohort(p, n_E, bz0, nb, Pcur);
+        nvtxRangePop();
+        if (rc) return rc;
+    }
+    CUDA_TRY(p, cudaEventRecord(p->ev[2], p->stream));
+    // failed energies -> NaN.  Lead failures (flags per energy) hit every device of that energy.
+    std::vector<int> h_status(batch), h_flags(n_E, 0);
+    fill_nan_kernel<<<(batch + 255) / 256, 256, 0, p->stream>>>(ptr<double>(p->T), ptr<int>(p->status), batch);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+    if (lead_open) CUDA_TRY(p, cudaMemcpyAsync(h_flags.data(), p->lead_flags.p, sizeof(int) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    int result = RGF_OK;
+    if (lead_open) {
+        std::vector<double> hT(batch);
+        CUDA_TRY(p, cudaMemcpy(hT.data(), p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToHost));
+        for (int b = 0; b < batch; b++) if (h_flags[b % n_E]) hT[b] = NAN;
+        CUDA_TRY(p, cudaMemcpy(p->T.p, hT.data(), sizeof(double) * (size_t)batch, cudaMemcpyHostToDevice));
+        result = fail(p, RGF_ENOCONV, "lead decimation did not converge in %d iterations for %d energies", kLeadMaxIt, lead_open);
+    }
+    for (int b = 0; b < batch; b++)
+        if (h_status[b]) { result = fail(p, RGF_ESINGULAR, "zero or non-finite pivot (first at batch item %d)", b); break; }
+    CUDA_TRY(p, cudaMemcpyAsync(T_out, p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaEventRecord(p->ev[3], p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    drain_update_events(p);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, p->ev[0], p->ev[3]); p->stats.ms_total = ms;
+    cudaEventElapsedTime(&ms, p->ev[0], p->ev[1]); p->stats.ms_leads = ms;
+    cudaEventElapsedTime(&ms, p->ev[1], p->ev[2]); p->stats.ms_sweep = ms;
+    cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_trace = ms + ms_trace;
+    return result;
+}
+
+int rgf_destroy(rgf_plan *p)
+{
+    if (!p) return RGF_OK;
+    cudaSetDevice(p->device);
+    if (p->stream) cudaStreamSynchronize(p->stream);
+    Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->counters,
+                   &p->G, &p->Nb, &p->Rb, &p->orig, &p->Pa, &p->Pb, &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha,
+                   &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4, &p->l_W, &p->stage_in, &p->stage_out};
+    for (Buf *b : bufs) release(*b);
+    for (auto &pr : p->upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+    for (int i = 0; i < 5; i++) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
+    delete p;
+    return RGF_OK;
+}
+
+const char *rgf_last_error(const rgf_plan *p) { return p ? p->err : kNoPlan; }
+
+int rgf_get_stats(const rgf_plan *p, rgf_stats *out)
+{
+    if (!p || !out) return RGF_EINVAL;
+    *out = p->stats;
+    return RGF_OK;
+}
+
+int rgf_set_profiling(rgf_plan *p, int level)
+{
+    if (!p || level < 0 || level > 1) return RGF_EINVAL;
+    p->profiling = level;
+    return RGF_OK;
+}
+
+int rgf_set_cohort(rgf_plan *p, int cohort)
+{
+    if (!p || cohort < 0) return RGF_EINVAL;
+    p->cohort_override = cohort;
+    return RGF_OK;
+}
+
+// FP64 tensor-pipe ceiling measured live: every warp issues independent DMMA.8x8x4 chains.
+__global__ void fp64_peak_kernel(double *out, int iters)
+{
+    double a = threadIdx.x * 1e-3, b = threadIdx.x * 2e-3;
+    double c[8][2];
+#pragma unroll
+    for (int j = 0; j < 8; j++) { c[j][0] = 0.0; c[j][1] = 0.0; }
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) dmma884(c[j][0], c[j][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; j++) s += c[j][0] + c[j][1];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+int rgf_fp64_peak_tflops(rgf_plan *p, double *tflops_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!tflops_out) return fail(p, RGF_EINVAL, "tflops_out is NULL");
+    int sms = 0;
+    CUDA_TRY(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
+    const int blocks = 2 * sms, threads = 512, iters = 40000;
+    if ((rc = ensure(p, p->stage_out, sizeof(double) * (size_t)blocks * threads))) return rc;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; rep++) {
+        CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
+        fp64_peak_kernel<<<blocks, threads, 0, p->stream>>>(ptr<double>(p->stage_out), iters);
+        CUDA_TRY(p, cudaEventRecord(p->ev[1], p->stream));
+        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        float ms = 0.f;
+        CUDA_TRY(p, cudaEventElapsedTime(&ms, p->ev[0], p->ev[1]));
+        double tf = (double)blocks * (threads / 32) * (double)iters * 8.0 * 512.0 / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    *tflops_out = best;
+    return RGF_OK;
+}
+
+int rgf_inverse_batched(rgf_plan *p, int n, int batch, const double *A, double *Ainv)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (n < 1 || batch < 1 || !A || !Ainv) return fail(p, RGF_EINVAL, "rgf_inverse_batched: bad argument");
+    memset(&p->stats, 0, sizeof(p->stats));
+    const size_t bytes = sizeof(cplx) * (size_t)n * n * batch;
+    if ((rc = ensure(p, p->stage_in, bytes))) return rc;
+    if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
+    if ((rc = ensure_inverse_ws(p, n, batch))) return rc;
+    CUDA_TRY(p, cudaMemcpyAsync(p->stage_in.p, A, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    if ((rc = run_inverse(p, ptr<cplx>(p->stage_in), n, batch, ptr<int>(p->status)))) return rc;
+    std::vector<int> h_status(batch);
+    CUDA_TRY(p, cudaMemcpyAsync(Ainv, p->stage_in.p, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    drain_update_events(p);
+    for (int b = 0; b < batch; b++)
+        if (h_status[b]) return fail(p, RGF_ESINGULAR, "zero or non-finite pivot in matrix %d", b);
+    return RGF_OK;
+}
+
+int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int side, double *Sigma_out,
+                         int *iterations_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_lead_self_energy before rgf_set_device");
+    if (dev < 0 || dev >= p->n_dev || (side != 1 && side != -1) || !Sigma_out) return fail(p, RGF_EINVAL, "bad argument");
+    memset(&p->stats, 0, sizeof(p->stats));
+    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
+    if ((rc = ensure(p, p->status, sizeof(int) * (size_t)n_E * p->n_dev))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)n_E * p->n_dev, p->stream));
+    int open = 0;
+    if ((rc = run_leads(p, n_E, eta, &open))) return rc;
+    const int M = p->M, L = p->L;
+    const size_t MM = (size_t)M * M;
+    std::vector<cplx> g(MM * n_E);
+    std::vector<uint8_t> m(M);
+    const cplx *src = side < 0 ? ptr<cplx>(p->gL) : lead_gR(p);
+    CUDA_TRY(p, cudaMemcpyAsync(g.data(), src, sizeof(cplx) * MM * n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(m.data(), ptr<uint8_t>(p->bond) + ((size_t)dev * (L + 1) + (side < 0 ? 0 : L)) * M, M,
+                                cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    // Sigma = t^2 m (.) g (.) m: the same masked scale the assembly kernel applies; done here on the
+    // host only to hand the checker a full matrix (this entry point is not on the hot path)
+    const double t2 = p->t * p->t;
+    for (int e = 0; e < n_E; e++)
+        for (int j = 0; j < M; j++)
+            for (int k = 0; k < M; k++) {
+                cplx &v = g[(size_t)e * MM + (size_t)j * M + k];
+                double s = (m[j] && m[k]) ? t2 : 0.0;
+                v.x *= s; v.y *= s;
+            }
+    CUDA_TRY(p, cudaMemcpy(Sigma_out, g.data(), sizeof(cplx) * MM * n_E, cudaMemcpyDefault));
+    if (iterations_out) *iterations_out = p->stats.lead_iterations;
+    if (open) return fail(p, RGF_ENOCONV, "lead decimation did not converge for %d energies", open);
+    return RGF_OK;
+}
+
+int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int precision, int nslices,
+                    double *g_out, double *P_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_sweep_state before rgf_set_device");
+    if (dev < 0 || dev >= p->n_dev || nslices < 1 || nslices > p->L || !g_out || !P_out) return fail(p, RGF_EINVAL, "bad argument");
+    if (precision != RGF_C128) return fail(p, RGF_EUNSUPPORTED, "only RGF_C128 is built in this version");
+    memset(&p->stats, 0, sizeof(p->stats));
+    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
+    const int batch = p->n_dev * n_E, M = p->M, nh = p->nh;
+    if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
+    if ((rc = ensure_sweep_ws(p, n_E))) return rc;
+    cplx *Pcur = nullptr;
+    if ((rc = run_sweep_cohort(p, n_E, eta, dev * n_E, n_E, nslices, &Pcur))) return rc;
+    const size_t bytes = sizeof(cplx) * (size_t)M * M * n_E;
+    if ((rc = ensure(p, p->stage_out, bytes))) return rc;
+    dim3 grid((unsigned)std::min((M * M + 255) / 256, 2048), n_E);
+    propagator_expand_kernel<<<grid, 256, 0, p->stream>>>(Pcur, ptr<cplx>(p->stage_out), M, nh, (nslices - 1) & 1);
+    CUDA_TRY(p, cudaGetLastError());
+    CUDA_TRY(p, cudaMemcpyAsync(g_out, p->G.p, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(P_out, p->stage_out.p, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    drain_update_events(p);
+    return RGF_OK;
+}
+
+}  // extern "C"

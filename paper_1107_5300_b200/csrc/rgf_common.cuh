@@ -1,0 +1,71 @@
+// rgf_common.cuh -- device helpers shared by the kernels of the RGF library (sm_100a only).
+// Complex numbers are double2 (x = re, y = im), interleaved, row-major everywhere in HBM.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rgf {
+
+typedef double2 cplx;
+
+__host__ __device__ __forceinline__ cplx cmake(double re, double im) { cplx r; r.x = re; r.y = im; return r; }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cmake(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return cmake(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b)
+{
+    return cmake(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+// c -= a*b
+__device__ __forceinline__ void cfnma(cplx &c, cplx a, cplx b)
+{
+    c.x = fma(-a.x, b.x, c.x); c.x = fma(a.y, b.y, c.x);
+    c.y = fma(-a.x, b.y, c.y); c.y = fma(-a.y, b.x, c.y);
+}
+__device__ __forceinline__ double cabs2(cplx a) { return fma(a.x, a.x, a.y * a.y); }
+// 1/a, scaled (Smith) so that |a|^2 cannot under/overflow for the magnitudes met here
+__device__ __forceinline__ cplx crecip(cplx a)
+{
+    if (fabs(a.x) >= fabs(a.y)) {
+        double r = a.y / a.x, d = fma(a.y, r, a.x);
+        double inv = 1.0 / d;
+        return cmake(inv, -r * inv);
+    } else {
+        double r = a.x / a.y, d = fma(a.x, r, a.y);
+        double inv = 1.0 / d;
+        return cmake(r * inv, -inv);
+    }
+}
+
+// ---- FP64 tensor core: mma.sync m8n8k4 (SASS: DMMA.8x8x4, the only native FP64 MMA shape on sm_100a)
+// Fragment ownership, lane = 4*g + t (g = lane>>2, t = lane&3):
+//   A (8x4, row): a  = A[g][t]        B (4x8, col): b = B[t][g]
+//   C (8x8):      c0 = C[g][2t], c1 = C[g][2t+1]
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// complex 8x8 += (8x4)*(4x8): 4 real DMMAs; nai = -a.im precomputed by the caller
+__device__ __forceinline__ void zmma884(double (&cre)[2], double (&cim)[2], double ar, double ai, double nai,
+                                        double br, double bi)
+{
+    dmma884(cre[0], cre[1], ar, br);
+    dmma884(cim[0], cim[1], ar, bi);
+    dmma884(cre[0], cre[1], nai, bi);
+    dmma884(cim[0], cim[1], ai, br);
+}
+
+// ---- cp.async (LDGSTS), 16 bytes = one complex128 element; src_bytes = 0 zero-fills
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src, int src_bytes)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem_src), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+// m_i[j] = 1 iff (i + j) even; bit test so that negative (lead) slice indices work
+__host__ __device__ __forceinline__ int mask_bit(int i, int j) { return (((i + j) & 1) == 0) ? 1 : 0; }
+
+}  // namespace rgf

@@ -1,0 +1,230 @@
+// sweep_kernels.cuh -- the O(M^2) kernels of the sweep: fused assembly of A_i (rows A1+A3 of
+// SURVEY.md 8a), compact start of the propagator, lead set-up/update kernels and the Gamma trace.
+//
+// Index conventions: batch item bz = d * n_E + e (device d, energy e).  Bond masks are bytes:
+//   bond[d][i+1][j] = m'_i[j]  for i = -1..L-1 (vacancy-aware inter-slice bond i <-> i+1)
+//   hop [d][i][j]   = 1 iff the intra-slice bond j <-> j+1 of slice i is alive
+// S_i = { j : (i + j) even } = { 2r + (i & 1) }: atoms of slice i bonded to slice i + 1.
+#pragma once
+#include "rgf_common.cuh"
+
+namespace rgf {
+
+// A_i = z I - H_i - t^2 m'_{i-1} (.) g_{i-1} (.) m'_{i-1}  [- Sigma_L if i = 0] [- Sigma_R if i = L-1],
+// written in place over g_{i-1} (Eq. 4 in the direct form; V = t diag(m) makes
+// V g V a masked scale, never a GEMM -- BASELINE.json:north_star item 2).
+__global__ void assemble_kernel(cplx *Gall, int M, int L, int i, int n_E, int bz0,
+                                const double *energies, double eta, double t,
+                                const double *onsite, const uint8_t *bond, const uint8_t *hop,
+                                const cplx *gL, const cplx *gR)
+{
+    const int bl = blockIdx.y;                 // index inside the cohort (G is cohort-local)
+    const int bz = bz0 + bl, d = bz / n_E, e = bz % n_E;
+    const long long MM = (long long)M * M;
+    cplx *G = Gall + (long long)bl * MM;
+    const double *eps = onsite + ((long long)d * L + i) * M;
+    const uint8_t *mprev = bond + ((long long)d * (L + 1) + i) * M;        // m'_{i-1}
+    const uint8_t *mlast = bond + ((long long)d * (L + 1) + L) * M;        // m'_{L-1}
+    const uint8_t *hp = hop + ((long long)d * L + i) * M;
+    const double t2 = t * t;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < MM;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int j = (int)(idx / M), k = (int)(idx % M);
+        cplx a = cmake(0.0, 0.0);
+        if (j == k) a = cmake(energies[e] - eps[j], eta);
+        else if (k == j + 1) { if (hp[j]) a.x = -t; }
+        else if (j == k + 1) { if (hp[k]) a.x = -t; }
+        if (mprev[j] && mprev[k]) {
+            // i = 0: previous "slice" is the left lead's surface slice -1
+            cplx gp = (i == 0) ? gL[(long long)e * MM + idx] : G[idx];
+            a.x -= t2 * gp.x; a.y -= t2 * gp.y;
+        }
+        if (i == L - 1 && mlast[j] && mlast[k]) {
+            cplx gr = gR[(long long)e * MM + idx];
+            a.x -= t2 * gr.x; a.y -= t2 * gr.y;
+        }
+        G[idx] = a;
+    }
+}
+
+// P_0 = g_0 restricted to rows S_0 and columns S_{-1} (compact nh x nh storage, ld = nh).
+__global__ void propagator_start_kernel(const cplx *Gall, cplx *Pall, int M, int nh)
+{
+    const int bl = blockIdx.y;
+    const cplx *G = Gall + (long long)bl * M * M;
+    cplx *P = Pall + (long long)bl * nh * nh;
+    const int nr = (M + 1) / 2, nc = M / 2;      // |S_0| (even j), |S_{-1}| (odd j)
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nr * nc; idx += gridDim.x * blockDim.x) {
+        int r = idx / nc, c = idx % nc;
+        P[(long long)r * nh + c] = G[(long long)(2 * r) * M + (2 * c + 1)];
+    }
+}
+
+// ---- lead decimation (Sancho-Rubio on the clean two-slice cell) -----------
+// Cell matrices are N x N, N = 2M: h00 = [[H_c, V_a],[V_a, H_c]], h01 = [[0,0],[V_b,0]].
+// alpha = h01 and beta = h01^T keep their block shape under alpha <- alpha g alpha,
+// beta <- beta g beta (only block (2,1) resp. (1,2) is ever non-zero), so only the M x M blocks
+// a = alpha[2,1] and b = beta[1,2] are stored and the products reduce to
+//   alpha g beta = [2,2] block  a g11 b      beta g alpha = [1,1] block  b g22 a
+//   alpha g alpha -> a g12 a                  beta g beta  -> b g21 b
+// which are the dense products with their structurally-zero terms left out.
+
+// W = z - X for dense N x N matrices per energy
+__global__ void lead_zminus_kernel(cplx *Wall, const cplx *Xall, int N, const double *energies, double eta)
+{
+    const int e = blockIdx.y;
+    const long long NN = (long long)N * N;
+    cplx *W = Wall + (long long)e * NN;
+    const cplx *X = Xall + (long long)e * NN;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < NN;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int j = (int)(idx / N), k = (int)(idx % N);
+        cplx x = X[idx];
+        cplx w = cmake(-x.x, -x.y);
+        if (j == k) { w.x += energies[e]; w.y += eta; }
+        W[idx] = w;
+    }
+}
+
+// eps = eps_s = h00; a = b = V_b.  va[j] = t m_pa[j], vb[j] = t m_pb[j] (m_p[j] = 1 iff (p + j) even)
+__global__ void lead_cell_init_kernel(cplx *eps_all, cplx *eps_s_all, cplx *a_all, cplx *b_all, int M, double t, int pa, int pb)
+{
+    const int e = blockIdx.y, N = 2 * M;
+    const long long NN = (long long)N * N, MM = (long long)M * M;
+    cplx *eps = eps_all + (long long)e * NN, *eps_s = eps_s_all + (long long)e * NN;
+    cplx *a = a_all + (long long)e * MM, *b = b_all + (long long)e * MM;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < NN;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int r = (int)(idx / N), c = (int)(idx % N);
+        int br = r >= M, bc = c >= M, j = r - br * M, k = c - bc * M;
+        double h;
+        if (br == bc) h = (j == k + 1 || k == j + 1) ? t : 0.0;
+        else h = (j == k) ? t * mask_bit(pa, j) : 0.0;
+        eps[idx] = cmake(h, 0.0);
+        eps_s[idx] = cmake(h, 0.0);
+        if (br == 0 && bc == 0) {
+            cplx v = cmake((j == k) ? t * mask_bit(pb, j) : 0.0, 0.0);
+            a[(long long)j * M + k] = v;
+            b[(long long)j * M + k] = v;
+        }
+    }
+}
+
+// eps[2,2] += agb; eps[1,1] += bga; eps_s += agb (right lead, side > 0) or bga (left lead)
+__global__ void lead_cell_accumulate_kernel(cplx *eps_all, cplx *eps_s_all, const cplx *agb_all, const cplx *bga_all, int M, int side)
+{
+    const int e = blockIdx.y, N = 2 * M;
+    const long long NN = (long long)N * N, MM = (long long)M * M;
+    cplx *eps = eps_all + (long long)e * NN, *eps_s = eps_s_all + (long long)e * NN;
+    const cplx *agb = agb_all + (long long)e * MM, *bga = bga_all + (long long)e * MM;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < MM;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int j = (int)(idx / M), k = (int)(idx % M);
+        long long i11 = (long long)j * N + k, i22 = (long long)(M + j) * N + (M + k);
+        cplx x = agb[idx], y = bga[idx];
+        eps[i22] = cadd(eps[i22], x);
+        eps[i11] = cadd(eps[i11], y);
+        if (side > 0) eps_s[i22] = cadd(eps_s[i22], x);
+        else eps_s[i11] = cadd(eps_s[i11], y);
+    }
+}
+
+// surface block of (z - eps_s)^-1: top-left (right lead) or bottom-right (left lead)
+__global__ void lead_extract_kernel(const cplx *g_all, cplx *out_all, int M, int side)
+{
+    const int e = blockIdx.y, N = 2 * M, off = side > 0 ? 0 : M;
+    const cplx *g = g_all + (long long)e * N * N;
+    cplx *out = out_all + (long long)e * M * M;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < (long long)M * M;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int j = (int)(idx / M), k = (int)(idx % M);
+        out[idx] = g[(long long)(off + j) * N + (off + k)];
+    }
+}
+
+// flags[e] = 1 if max(|alpha|, |beta|) >= tol for energy e; *n_open counts them
+__global__ void lead_converged_kernel(const cplx *alpha, const cplx *beta, int M, double tol, int *flags, int *n_open)
+{
+    const int e = blockIdx.x;
+    const long long MM = (long long)M * M, off = (long long)e * MM;
+    double m = 0.0;
+    for (long long idx = threadIdx.x; idx < MM; idx += blockDim.x) {
+        double a = cabs2(alpha[off + idx]), b = cabs2(beta[off + idx]);
+        a = a > b ? a : b;
+        if (!(a <= m)) m = a;          // NaN propagates as "not converged"
+    }
+    __shared__ double red[32];
+    for (int o = 16; o > 0; o >>= 1) { double x = __shfl_xor_sync(0xffffffffu, m, o); if (!(x <= m)) m = x; }
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); w++) if (!(red[w] <= m)) m = red[w];
+        int open = !(m < tol * tol);
+        flags[e] = open;
+        if (open) atomicAdd(n_open, 1);
+    }
+}
+
+// ---- trace -------------------------------------------------------------
+// Gamma = i (Sigma - Sigma^dagger) = -2 Im Sigma (Sigma is complex symmetric), Sigma = t^2 m (.) g (.) m.
+// GamR compact on S_{L-1} x S_{L-1}: GamR[r][r'] = -2 t^2 m[jr] m[jr'] Im gR[e][jr][jr'], jr = 2r + pR.
+__global__ void gamma_right_kernel(cplx *GamAll, const cplx *gR, const uint8_t *bond, int M, int L, int nh, int n_E, int bz0, double t)
+{
+    const int bl = blockIdx.y, bz = bz0 + bl, d = bz / n_E, e = bz % n_E;
+    const int pR = (L - 1) & 1, nr = (M - pR + 1) / 2;
+    const uint8_t *m = bond + ((long long)d * (L + 1) + L) * M;
+    cplx *Gam = GamAll + (long long)bl * nh * nh;
+    const cplx *g = gR + (long long)e * M * M;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nr * nr; idx += gridDim.x * blockDim.x) {
+        int r = idx / nr, c = idx % nr, jr = 2 * r + pR, jc = 2 * c + pR;
+        double v = (m[jr] && m[jc]) ? -2.0 * t * t * g[(long long)jr * M + jc].y : 0.0;
+        Gam[(long long)r * nh + c] = cmake(v, 0.0);
+    }
+}
+
+// T = Re sum_{c,c'} GamL[c][c'] Y[c'][c],  Y = P^dagger GamR P (nc x nc, ld = nh), GamL real, on S_{-1} (odd j).
+__global__ void trace_kernel(const cplx *Yall, const cplx *gL, const uint8_t *bond, int M, int L, int nh, int n_E, int bz0,
+                             double t, double *T_out)
+{
+    const int bl = blockIdx.x, bz = bz0 + bl, d = bz / n_E, e = bz % n_E;
+    const int nc = M / 2;
+    const uint8_t *m = bond + ((long long)d * (L + 1) + 0) * M;    // m'_{-1}
+    const cplx *Y = Yall + (long long)bl * nh * nh;
+    const cplx *g = gL + (long long)e * M * M;
+    double acc = 0.0;
+    for (int idx = threadIdx.x; idx < nc * nc; idx += blockDim.x) {
+        int c = idx / nc, c2 = idx % nc, j = 2 * c + 1, j2 = 2 * c2 + 1;
+        if (m[j] && m[j2]) acc += (-2.0 * t * t * g[(long long)j * M + j2].y) * Y[(long long)c2 * nh + c].x;
+    }
+    __shared__ double red[32];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) T_out[bz] = v;
+    }
+}
+
+// expand the compact propagator into a full M x M matrix (NaN where not propagated), for rgf_sweep_state
+__global__ void propagator_expand_kernel(const cplx *Pall, cplx *Out, int M, int nh, int pi)
+{
+    const int bl = blockIdx.y;
+    const cplx *P = Pall + (long long)bl * nh * nh;
+    cplx *O = Out + (long long)bl * M * M;
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < M * M; idx += gridDim.x * blockDim.x) {
+        int j = idx / M, k = idx % M;
+        bool have = ((j & 1) == pi) && ((k & 1) == 1);
+        O[idx] = have ? P[(long long)(j >> 1) * nh + (k >> 1)] : cmake(nan, nan);
+    }
+}
+
+__global__ void fill_nan_kernel(double *T, const int *status, int n)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && status[i]) T[i] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
+}  // namespace rgf

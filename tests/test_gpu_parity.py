@@ -1,0 +1,185 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerance (BASELINE.json:north_star): complex128 |dT| <= 1e-9 * max(1, T).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1107_5300_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def rgf():
+    from paper_1107_5300_b200 import binding
+    return binding
+
+
+@pytest.fixture()
+def plan(rgf):
+    with rgf.Plan(0) as p:
+        yield p
+
+
+def tol(T):
+    return 1e-9 * np.maximum(1.0, np.abs(T))
+
+
+# ---- A4: the batched inverse on its own -----------------------------------------------------
+
+@pytest.mark.parametrize("n,batch", [(1, 3), (5, 4), (20, 7), (32, 2), (33, 3), (64, 2), (100, 5), (244, 6), (256, 2), (300, 2), (600, 1)])
+def test_inverse_batched_matches_oracle_and_lapack(rgf, plan, oracle, n, batch):
+    rng = np.random.default_rng(n * 31 + batch)
+    A = rng.standard_normal((batch, n, n)) + 1j * rng.standard_normal((batch, n, n))
+    A[0] += np.diag(np.zeros(n))
+    if n >= 5:
+        A[-1, 0, 0] = 0.0            # forces a row exchange in the first column
+        A[-1, 3, 3] = 0.0
+    out = np.empty_like(A)
+    rgf.rgf_inverse_batched(plan.handle, n, batch, A, out)
+    for b in range(batch):
+        ref = np.linalg.inv(A[b])
+        scale = np.max(np.abs(ref))
+        assert np.max(np.abs(out[b] - ref)) < 1e-9 * scale, (b, np.max(np.abs(out[b] - ref)) / scale)
+        assert np.max(np.abs(A[b] @ out[b] - np.eye(n))) < 1e-8
+    if n <= 100:
+        assert np.max(np.abs(out[0] - oracle.inverse(A[0]))) < 1e-9 * np.max(np.abs(out[0]))
+
+
+def test_inverse_of_actual_slice_matrix(rgf, plan, oracle):
+    """A_i = z - H_i - Sigma of a disordered M=244 slice: complex symmetric, tiny imaginary part."""
+    M = 244
+    rng = np.random.default_rng(5)
+    on = rng.uniform(-0.1, 0.1, M)
+    A = np.zeros((3, M, M), dtype=complex)
+    for b, E in enumerate((0.013, 0.5, -0.97)):
+        A[b] = np.diag(E + 1e-9j - on) - np.diag(np.full(M - 1, -2.7), 1) - np.diag(np.full(M - 1, -2.7), -1)
+    out = np.empty_like(A)
+    rgf.rgf_inverse_batched(plan.handle, M, 3, A, out)
+    for b in range(3):
+        ref = oracle.inverse(A[b])
+        assert np.max(np.abs(out[b] - ref)) < 1e-9 * np.max(np.abs(ref))
+
+
+def test_singular_matrix_is_reported(rgf, plan):
+    A = np.zeros((2, 8, 8), dtype=complex)
+    A[0] = np.eye(8)
+    out = np.empty_like(A)
+    with pytest.raises(rgf.RgfError) as e:
+        rgf.rgf_inverse_batched(plan.handle, 8, 2, A, out)
+    assert e.value.code == rgf.RGF_ESINGULAR
+
+
+# ---- A2: lead self-energies -----------------------------------------------------------------
+
+@pytest.mark.parametrize("M,L", [(20, 40), (20, 41), (7, 5), (64, 10)])
+def test_lead_self_energy_matches_oracle(rgf, plan, oracle, M, L):
+    E = np.array([-2.0, -0.4, 0.013, 0.8, 1.7])
+    vac = np.zeros((L, M), dtype=np.uint8)
+    vac[0, 1] = 1
+    vac[L - 1, 2 if (L - 1) % 2 == 0 else 3] = 1
+    on = np.zeros((L, M))
+    plan.set_device(on, -2.7, vac)
+    for side in (-1, +1):
+        S = np.empty((len(E), M, M), dtype=complex)
+        it = rgf.rgf_lead_self_energy(plan.handle, 0, E, len(E), 1e-9, side, S)
+        assert 20 <= it <= 64
+        for k, e in enumerate(E):
+            ref, _ = oracle.lead_self_energy(M, L, vac, -2.7, e, 1e-9, side)
+            assert np.max(np.abs(S[k] - ref)) < 1e-9 * max(1.0, np.max(np.abs(ref))), (side, e)
+
+
+# ---- A3-A5: state of the sweep ---------------------------------------------------------------
+
+@pytest.mark.parametrize("M,L,ns", [(20, 12, 1), (20, 12, 2), (20, 12, 7), (21, 9, 9), (64, 6, 5)])
+def test_sweep_state_matches_oracle(rgf, plan, oracle, M, L, ns):
+    on = inputs.anderson(M, L, 0.25, 99 + M)
+    plan.set_device(on, -2.7)
+    E = np.array([-1.1, 0.07, 0.9])
+    g = np.empty((3, M, M), dtype=complex)
+    P = np.empty((3, M, M), dtype=complex)
+    rgf.rgf_sweep_state(plan.handle, 0, E, 3, 1e-9, rgf.RGF_C128, ns, g, P)
+    for k, e in enumerate(E):
+        g0, P0 = oracle.sweep_state(on, None, -2.7, e, 1e-9, ns)
+        assert np.max(np.abs(g[k] - g0)) < 1e-9 * np.max(np.abs(g0))
+        have = ~np.isnan(P[k].real)
+        rows = (np.arange(M) % 2) == ((ns - 1) % 2)
+        cols = (np.arange(M) % 2) == 1
+        assert np.array_equal(have, np.outer(rows, cols))
+        assert np.max(np.abs(P[k][have] - P0[have])) < 1e-9 * max(1e-300, np.max(np.abs(P0)))
+
+
+# ---- end to end ----------------------------------------------------------------------------
+
+def test_config0_matches_oracle_and_closed_form(rgf, plan, oracle):
+    from test_oracle_pins import closed_form_T
+    w = inputs.config0()
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)[0]
+    T_or = oracle.transmission_batch(w.onsite[0], None, w.t, w.energies, w.eta)
+    assert np.all(np.abs(T - T_or) <= tol(T_or)), np.max(np.abs(T - T_or))
+    for e, tk in zip(w.energies, T):
+        assert abs(tk - closed_form_T(w.M, w.L, e)[0]) < 1e-8
+    assert plan.stats()["launches"] > 0
+
+
+@pytest.mark.parametrize("M,L,W", [(20, 1, 0.2), (20, 2, 0.2), (21, 17, 0.3), (50, 33, 0.25), (128, 24, 0.25)])
+def test_disordered_small_matches_oracle(rgf, plan, oracle, M, L, W):
+    on = inputs.anderson(M, L, W, 1000 + M + L)
+    E = np.linspace(-1.0, 1.0, 8)
+    plan.set_device(on, -2.7)
+    T = plan.transmission(E, 1e-9)[0]
+    T_or = oracle.transmission_batch(on, None, -2.7, E, 1e-9)
+    assert np.all(np.abs(T - T_or) <= tol(T_or)), np.max(np.abs(T - T_or))
+
+
+def test_batched_devices_vacancies_and_cohorts(rgf, plan, oracle):
+    """4 devices batched (configs[1] shape, reduced), one with edge vacancies; ragged cohorts."""
+    M, L = 32, 20
+    on = np.stack([inputs.anderson(M, L, 0.25, s) for s in (1107, 1108, 1109)])
+    vac = np.zeros((3, L, M), dtype=np.uint8)
+    vac[2] = inputs.edge_vacancies(M, L, 0.3, 5303)
+    vac[2, 0, 1] = 1
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.linspace(-1.0, 1.0, 8)          # even count: E = 0 (a resonance of the isolated lead cell) is not sampled
+    plan.set_device(on, -2.7, vac)
+    T_ref = np.stack([oracle.transmission_batch(on[d], vac[d], -2.7, E, 1e-9) for d in range(3)])
+    for cohort in (0, 5, 21, 4):
+        rgf.rgf_set_cohort(plan.handle, cohort)
+        T = plan.transmission(E, 1e-9)
+        assert T.shape == (3, 8)
+        assert np.all(np.abs(T - T_ref) <= tol(T_ref)), (cohort, np.max(np.abs(T - T_ref)))
+
+
+def test_device_pointers(rgf, plan, oracle):
+    import torch
+    w = inputs.config0(n_E=16)
+    plan.set_device(w.onsite, w.t)
+    E = torch.tensor(w.energies, dtype=torch.float64, device="cuda")
+    T = torch.empty(16, dtype=torch.float64, device="cuda")
+    rgf.rgf_transmission(plan.handle, E, 16, w.eta, rgf.RGF_C128, T)
+    T_or = oracle.transmission_batch(w.onsite[0], None, w.t, w.energies, w.eta)
+    assert np.all(np.abs(T.cpu().numpy() - T_or) <= tol(T_or))
+
+
+def test_errors(rgf, plan):
+    E = np.array([0.1])
+    T = np.empty(1)
+    with pytest.raises(rgf.RgfError) as e:
+        rgf.rgf_transmission(plan.handle, E, 1, 1e-9, rgf.RGF_C128, T)
+    assert e.value.code == rgf.RGF_ESTATE
+    plan.set_device(np.zeros((4, 6)), -2.7)
+    for bad in (dict(eta=0.0), dict(eta=-1.0)):
+        with pytest.raises(rgf.RgfError) as e:
+            rgf.rgf_transmission(plan.handle, E, 1, bad["eta"], rgf.RGF_C128, T)
+        assert e.value.code == rgf.RGF_EINVAL
+    with pytest.raises(rgf.RgfError) as e:
+        rgf.rgf_transmission(plan.handle, np.array([np.nan]), 1, 1e-9, rgf.RGF_C128, T)
+    assert e.value.code == rgf.RGF_EINVAL
+    with pytest.raises(rgf.RgfError) as e:
+        rgf.rgf_set_device(plan.handle, 1, 4, np.zeros((4, 1)), -2.7)
+    assert e.value.code == rgf.RGF_EINVAL
