@@ -168,201 +168,6 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
 }
 
 // ------------------------------------------------------------------------------------------
-// Panel factorisation, two-level (n <= 256, B = 32): the n x 32 panel lives in shared memory;
-// it is processed in 4 sub-blocks of 8 columns.  Inside a sub-block each thread keeps the 8
-// entries of its row in registers and the 8 pivot steps are rank-1 updates of those 8 columns
-// only (DFMA); the other 24 panel columns then get the sub-block's transform as one
-// (n x 8) x (8 x 24) product on the FP64 tensor pipe.  Rows are not moved inside the panel
-// (implicit pivoting); the exchanges are made physical when the panel is written back.
-// ------------------------------------------------------------------------------------------
-constexpr int P2_B = 32, P2_SB = 8, P2_NT = 256;
-constexpr int P2_LDP = P2_B + 4;      // 36: C/A fragment loads conflict-free
-constexpr int P2_LDM = P2_SB + 4;     // 12
-constexpr int P2_LDR = P2_B + 2;      // 34
-__host__ __device__ constexpr size_t gj_panel2_smem(int n)
-{
-    return sizeof(cplx) * ((size_t)P2_NT * P2_LDP + (size_t)P2_NT * P2_LDM + P2_SB * P2_LDR + P2_SB) +
-           sizeof(double) * 32 + sizeof(int) * (32 + 2 * (size_t)n + P2_B + 2 * P2_B + 4) + 64;
-}
-static_assert(P2_NT * P2_LDM >= 2 * P2_B * GJ_CH, "row-move staging aliases the multiplier buffer");
-
-__global__ void __launch_bounds__(P2_NT) gj_panel2_kernel(cplx *Gall, long long g_batch, int n, int k0,
-                                                           cplx *Nall, cplx *Rall, int *origall, int *status)
-{
-    constexpr int B = P2_B, SB = P2_SB, NT = P2_NT, LDP = P2_LDP, LDM = P2_LDM, LDR = P2_LDR;
-    extern __shared__ __align__(16) unsigned char gj_smem[];
-    cplx *panel = reinterpret_cast<cplx *>(gj_smem);           // [NT][LDP], original row order
-    cplx *mult = panel + NT * LDP;                              // [NT][LDM]  N'_s - E_s
-    cplx *Rs = mult + NT * LDM;                                 // [SB][LDR]  pivot rows of the sub-block
-    cplx *pivrow = Rs + SB * LDR;                               // [SB]
-    cplx *stage = mult;                                         // [2B][GJ_CH], used after the factorisation only
-    double *red_val = reinterpret_cast<double *>(pivrow + SB);
-    int *red_idx = reinterpret_cast<int *>(red_val + 32);
-    int *rowAt = red_idx + 32;
-    int *posOf = rowAt + n;
-    int *prow = posOf + n;                                      // [B] pivot row of each panel column
-    int *moved = prow + B;
-    int *nmoved = moved + 2 * B;
-
-    const int b = blockIdx.x;
-    cplx *G = Gall + (long long)b * g_batch;
-    cplx *Nbuf = Nall + (long long)b * n * B;
-    cplx *Rbuf = Rall + (long long)b * n * B;
-    int *orig = origall + (long long)b * n;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-    const int r = tid;
-    const bool has_row = r < n;
-    const int bw = (n - k0 < B) ? (n - k0) : B;
-
-    // ---- load the panel (coalesced: 32 consecutive lanes read one row's 512 bytes)
-    for (int e = tid; e < NT * B; e += NT) {
-        int rr = e / B, c = e % B;
-        panel[rr * LDP + c] = (rr < n && c < bw) ? G[(long long)rr * n + k0 + c] : cmake(0.0, 0.0);
-    }
-    for (int i = tid; i < n; i += NT) { rowAt[i] = i; posOf[i] = i; }
-    bool used = (!has_row || r < k0);
-    __syncthreads();
-
-    for (int s = 0; s < B / SB; s++) {
-        const int c0 = s * SB;
-        const int ncols = bw - c0 < SB ? bw - c0 : SB;
-        if (ncols <= 0) break;
-        cplx row[SB];
-#pragma unroll
-        for (int j = 0; j < SB; j++) row[j] = panel[r * LDP + c0 + j];
-#pragma unroll 1
-        for (int cc = 0; cc < ncols; cc++) {
-            cplx x = row[0];
-#pragma unroll
-            for (int j = 1; j < SB; j++) if (j == cc) x = row[j];
-            double v = used ? -1.0 : cabs2(x);
-            if (!(v == v)) v = 1e300;
-            int idx = r;
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                double ov = __shfl_xor_sync(0xffffffffu, v, off);
-                int oi = __shfl_xor_sync(0xffffffffu, idx, off);
-                if (ov > v || (ov == v && oi < idx)) { v = ov; idx = oi; }
-            }
-            if (lane == 0) { red_val[warp] = v; red_idx[warp] = idx; }
-            __syncthreads();
-            double bv = red_val[0]; int pr = red_idx[0];
-#pragma unroll
-            for (int w = 1; w < NT / 32; w++) {
-                double ov = red_val[w]; int oi = red_idx[w];
-                if (ov > bv || (ov == bv && oi < pr)) { bv = ov; pr = oi; }
-            }
-            if (r == pr) {
-                if (!(bv > 0.0) || !(bv < 1e299)) status[b] = 1;
-                double iv = 1.0 / bv;                       // 1/x = conj(x) / |x|^2
-                cplx d = cmake(x.x * iv, -x.y * iv);
-#pragma unroll
-                for (int j = 0; j < SB; j++) {
-                    cplx y = (j == cc) ? cmake(1.0, 0.0) : row[j];
-                    row[j] = cmul(y, d);
-                    pivrow[j] = row[j];
-                }
-                used = true;
-                int k = k0 + c0 + cc, a = rowAt[k], pp = posOf[pr];
-                rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
-                prow[c0 + cc] = pr;
-            }
-            __syncthreads();
-            if (r != pr) {
-#pragma unroll
-                for (int j = 0; j < SB; j++) {
-                    cplx y = (j == cc) ? cmake(0.0, 0.0) : row[j];
-                    cfnma(y, x, pivrow[j]);
-                    row[j] = y;
-                }
-            }
-        }
-        __syncthreads();
-        // ---- N'_s back to the panel, multipliers N'_s - E_s, snapshot of the pivot rows
-#pragma unroll
-        for (int j = 0; j < SB; j++) {
-            panel[r * LDP + c0 + j] = row[j];
-            cplx m = row[j];
-            if (j < ncols && prow[c0 + j] == r) m.x -= 1.0;
-            mult[r * LDM + j] = m;
-        }
-        for (int e = tid; e < SB * B; e += NT) {
-            int k = e / B, c = e % B;
-            Rs[k * LDR + c] = (k < ncols) ? panel[prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
-        }
-        __syncthreads();
-        // ---- other panel columns: panel[:, J] += mult (n x 8) * Rs[:, J] (8 x |J|) on DMMA
-        const int nbmax = (bw + 7) / 8;
-        for (int nb = 0; nb < nbmax; nb++) {
-            if (nb == s) continue;
-            double cre[4][2], cim[4][2];
-            cplx *Cw = panel + (warp * 32) * LDP + nb * 8;
-#pragma unroll
-            for (int i = 0; i < 4; i++) {
-                cplx v0 = Cw[(i * 8 + g) * LDP + 2 * t], v1 = Cw[(i * 8 + g) * LDP + 2 * t + 1];
-                cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
-            }
-#pragma unroll
-            for (int kk = 0; kk < SB; kk += 4) {
-                cplx bb = Rs[(kk + t) * LDR + nb * 8 + g];
-#pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    cplx a = mult[(warp * 32 + i * 8 + g) * LDM + kk + t];
-                    zmma884(cre[i], cim[i], a.x, a.y, -a.y, bb.x, bb.y);
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < 4; i++) {
-                Cw[(i * 8 + g) * LDP + 2 * t] = cmake(cre[i][0], cim[i][0]);
-                Cw[(i * 8 + g) * LDP + 2 * t + 1] = cmake(cre[i][1], cim[i][1]);
-            }
-        }
-        __syncthreads();
-    }
-
-    // ---- list of positions whose row changed
-    if (tid == 0) *nmoved = 0;
-    __syncthreads();
-    for (int i = tid; i < n; i += NT)
-        if (rowAt[i] != i) { int q = atomicAdd(nmoved, 1); moved[q] = i; }
-    __syncthreads();
-    const int nm = *nmoved;                      // <= 2B
-
-    // ---- new panel columns and multipliers, written in exchanged (physical) row order
-    for (int e = tid; e < n * B; e += NT) {
-        int pos = e / B, c = e % B;
-        cplx v = panel[rowAt[pos] * LDP + c];
-        if (c < bw) G[(long long)pos * n + k0 + c] = v;
-        if (pos == k0 + c) v.x -= 1.0;
-        Nbuf[(long long)pos * B + c] = v;
-    }
-    // ---- origin bookkeeping: orig[pos] <- orig[rowAt[pos]]
-    int my_orig = 0;
-    if (tid < nm) my_orig = orig[rowAt[moved[tid]]];
-    __syncthreads();
-    if (tid < nm) orig[moved[tid]] = my_orig;
-
-    // ---- move the exchanged rows in all non-panel columns, chunk by chunk
-    for (int j0 = 0; j0 < n; j0 += GJ_CH) {
-        for (int e = tid; e < nm * GJ_CH; e += NT) {
-            int q = e / GJ_CH, j = j0 + e % GJ_CH;
-            if (j < n && (j < k0 || j >= k0 + B)) stage[q * GJ_CH + (j - j0)] = G[(long long)rowAt[moved[q]] * n + j];
-        }
-        __syncthreads();
-        for (int e = tid; e < nm * GJ_CH; e += NT) {
-            int q = e / GJ_CH, j = j0 + e % GJ_CH;
-            if (j < n && (j < k0 || j >= k0 + B)) G[(long long)moved[q] * n + j] = stage[q * GJ_CH + (j - j0)];
-        }
-        __syncthreads();
-    }
-    // ---- pivot rows (after the exchange, before the update) for the update kernel
-    for (int e = tid; e < B * n; e += NT) {
-        int c = e / n, j = e % n;
-        Rbuf[(long long)c * n + j] = (c < bw) ? G[(long long)(k0 + c) * n + j] : cmake(0.0, 0.0);
-    }
-}
-
-// ------------------------------------------------------------------------------------------
 // Trailing update on the FP64 tensor pipe: G[:,J] += Nbuf (n x B) * Rbuf[:,J] (B x |J|).
 // CTA = 4 warps stacked on rows: tile 128 rows x 32 columns; the accumulators are initialised
 // from G and stored back in place (each element is read and written by exactly one lane).

@@ -1,0 +1,290 @@
+// gj_inverse32.cuh -- the fast path of the batched complex128 inverse for n <= 256 (the paper's
+// 30 nm ribbon is n = 244): blocked Gauss-Jordan with partial pivoting, panels of 32 columns,
+// ping-pong buffers X -> Y so that row exchanges cost nothing.
+//
+// One panel step k (columns K = [k0, k0+32)), for every matrix of the batch:
+//   gj32_panel_kernel : reads X[:, K]; Gauss-Jordan with partial pivoting on the n x 32 panel held
+//                       in shared memory (4 sub-blocks of 8 columns: rank-1 DFMA updates inside the
+//                       sub-block with the thread's row in registers, then one (n x 8) x (8 x 24)
+//                       DMMA product for the other panel columns).  Rows are never moved; the
+//                       exchange is the map rowAt[pos] = row of X that belongs at position pos.
+//                       Writes Y[pos, K] = N'[rowAt[pos], :], Mult[pos, :] = N' - E, rowAt, orig.
+//   gj32_update_kernel: Y[pos, J] = X[rowAt[pos], J] + Mult[pos, :] * X[rowAt[k0 + :], J]   (FP64 DMMA)
+// then X <-> Y.  After the last panel gj32_unpermute_kernel scatters columns: out[:, orig[pos]] = X[:, pos].
+// (Eq. 4 / PAPER.md:53 "one call of the linear equation solver".)
+#pragma once
+#include "rgf_common.cuh"
+
+namespace rgf {
+
+constexpr int G32_B = 32, G32_SB = 8, G32_NT = 256;
+constexpr int G32_LDP = G32_B + 4;      // 36: A / C fragment accesses conflict-free
+constexpr int G32_LDR = G32_B + 2;      // 34
+__host__ __device__ constexpr size_t gj32_panel_smem(int n)
+{
+    return sizeof(cplx) * ((size_t)G32_NT * G32_LDP + G32_SB * G32_LDR + G32_SB) + sizeof(unsigned long long) * 32 +
+           sizeof(int) * (2 * (size_t)n + G32_B + 8) + 64;
+}
+
+__global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restrict__ Xall, cplx *__restrict__ Yall, long long g_batch,
+                                                            int n, int k0, cplx *__restrict__ Mall, int *__restrict__ rowAtAll,
+                                                            int *__restrict__ origall, int *__restrict__ status)
+{
+    constexpr int B = G32_B, SB = G32_SB, NT = G32_NT, LDP = G32_LDP, LDR = G32_LDR;
+    extern __shared__ __align__(16) unsigned char gj_smem[];
+    cplx *panel = reinterpret_cast<cplx *>(gj_smem);           // [NT][LDP], rows in X order
+    cplx *Rs = panel + NT * LDP;                                // [SB][LDR] pivot rows of the sub-block
+    cplx *pivrow = Rs + SB * LDR;                               // [SB]
+    unsigned long long *red = reinterpret_cast<unsigned long long *>(pivrow + SB);   // [32]
+    int *rowAt = reinterpret_cast<int *>(red + 32);
+    int *posOf = rowAt + n;
+    int *prow = posOf + n;                                      // [B]
+
+    const int b = blockIdx.x;
+    const cplx *X = Xall + (long long)b * g_batch;
+    cplx *Y = Yall + (long long)b * g_batch;
+    cplx *Mult = Mall + (long long)b * n * B;
+    int *orig = origall + (long long)b * n;
+    int *rowAtG = rowAtAll + (long long)b * n;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const int r = tid;
+    const bool has_row = r < n;
+    const int bw = (n - k0 < B) ? (n - k0) : B;
+
+    // ---- panel -> shared memory: one warp per row segment of 512 bytes, all copies in flight at once
+    for (int e = tid; e < NT * B; e += NT) {
+        int rr = e / B, c = e % B;
+        bool ok = rr < n && c < bw;
+        cp_async16(panel + rr * LDP + c, ok ? X + (long long)rr * n + k0 + c : X, ok ? 16 : 0);
+    }
+    cp_async_commit();
+    for (int i = tid; i < n; i += NT) { rowAt[i] = i; posOf[i] = i; }
+    bool used = (!has_row || r < k0);          // positions < k0 hold the pivot rows of earlier panels
+    cp_async_wait<0>();
+    __syncthreads();
+
+    for (int s = 0; s < B / SB; s++) {
+        const int c0 = s * SB;
+        const int ncols = bw - c0 < SB ? bw - c0 : SB;
+        if (ncols <= 0) break;
+        cplx row[SB];
+#pragma unroll
+        for (int j = 0; j < SB; j++) row[j] = panel[r * LDP + c0 + j];
+#pragma unroll 1
+        for (int cc = 0; cc < ncols; cc++) {
+            cplx x = row[0];
+#pragma unroll
+            for (int j = 1; j < SB; j++) if (j == cc) x = row[j];
+            // ---- pivot search.  Key = (high 32 bits of |x|^2, ~row): the maximum over the block is a
+            // pivot within 2^-20 of the largest magnitude (any such pivot is as good), lowest row on ties.
+            const double v = cabs2(x);
+            unsigned hi = used ? 0u : (unsigned)__double2hiint(v);
+            if (!used && !(v == v)) hi = 0x7ff80000u;                 // NaN: report it
+            const unsigned wmax = __reduce_max_sync(0xffffffffu, hi);
+            const unsigned ball = __ballot_sync(0xffffffffu, hi == wmax);
+            if (lane == 0) red[warp] = ((unsigned long long)wmax << 32) | (unsigned)(0xffffffffu - (unsigned)(warp * 32 + __ffs(ball) - 1));
+            __syncthreads();
+            unsigned long long best = red[0];
+#pragma unroll
+            for (int w = 1; w < NT / 32; w++) { unsigned long long o = red[w]; best = o > best ? o : best; }
+            const int pr = (int)(0xffffffffu - (unsigned)(best & 0xffffffffu));
+            if (r == pr) {
+                const unsigned bh = (unsigned)(best >> 32);
+                if (bh == 0u || bh >= 0x7ff00000u) status[b] = 1;     // zero / non-finite pivot
+                const double iv = 1.0 / v;                             // 1/x = conj(x) / |x|^2
+                const cplx d = cmake(x.x * iv, -x.y * iv);
+#pragma unroll
+                for (int j = 0; j < SB; j++) {
+                    cplx y = (j == cc) ? cmake(1.0, 0.0) : row[j];
+                    row[j] = cmul(y, d);
+                    pivrow[j] = row[j];
+                }
+                used = true;
+                const int k = k0 + c0 + cc, a = rowAt[k], pp = posOf[pr];
+                rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
+                prow[c0 + cc] = pr;
+            }
+            __syncthreads();
+            if (r != pr) {
+#pragma unroll
+                for (int j = 0; j < SB; j++) {
+                    cplx y = (j == cc) ? cmake(0.0, 0.0) : row[j];
+                    cfnma(y, x, pivrow[j]);
+                    row[j] = y;
+                }
+            }
+        }
+        __syncthreads();
+        // ---- N'_s back to the panel; snapshot of the sub-block's pivot rows (their other columns)
+#pragma unroll
+        for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
+        for (int e = tid; e < SB * B; e += NT) {
+            int k = e / B, c = e % B;
+            if (c < c0 || c >= c0 + SB) Rs[k * LDR + c] = (k < ncols) ? panel[prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
+        }
+        __syncthreads();
+        // ---- other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs[:, J] (8 x |J|) on DMMA
+        const int nbmax = (bw + 7) / 8;
+        if (nbmax > 1) {
+            int pk[2];
+#pragma unroll
+            for (int q = 0; q < 2; q++) pk[q] = (q * 4 + t < ncols) ? prow[c0 + q * 4 + t] : -1;
+            cplx a[2][4];
+#pragma unroll
+            for (int q = 0; q < 2; q++)
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    const int rr = warp * 32 + i * 8 + g;
+                    a[q][i] = panel[rr * LDP + c0 + q * 4 + t];
+                    if (rr == pk[q]) a[q][i].x -= 1.0;
+                }
+            for (int nb = 0; nb < nbmax; nb++) {
+                if (nb == s) continue;
+                double cre[4][2], cim[4][2];
+                cplx *Cw = panel + (warp * 32) * LDP + nb * 8;
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    cplx v0 = Cw[(i * 8 + g) * LDP + 2 * t], v1 = Cw[(i * 8 + g) * LDP + 2 * t + 1];
+                    cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
+                }
+#pragma unroll
+                for (int q = 0; q < 2; q++) {
+                    cplx bb = Rs[(q * 4 + t) * LDR + nb * 8 + g];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) zmma884(cre[i], cim[i], a[q][i].x, a[q][i].y, -a[q][i].y, bb.x, bb.y);
+                }
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    Cw[(i * 8 + g) * LDP + 2 * t] = cmake(cre[i][0], cim[i][0]);
+                    Cw[(i * 8 + g) * LDP + 2 * t + 1] = cmake(cre[i][1], cim[i][1]);
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- outputs, in exchanged (position) order
+    for (int e = tid; e < n * B; e += NT) {
+        int pos = e / B, c = e % B;
+        cplx v = panel[rowAt[pos] * LDP + c];
+        if (c < bw) Y[(long long)pos * n + k0 + c] = v;
+        if (pos == k0 + c) v.x -= 1.0;
+        Mult[(long long)pos * B + c] = v;
+    }
+    // orig[pos] <- orig[rowAt[pos]]; rowAt for the update kernel
+    int o = 0;
+    if (has_row) o = orig[rowAt[r]];
+    __syncthreads();
+    if (has_row) { orig[r] = o; rowAtG[r] = rowAt[r]; }
+}
+
+// ------------------------------------------------------------------------------------------
+// Y[pos, J] = X[rowAt[pos], J] + Mult[pos, :] (n x 32) * X[rowAt[k0 + :], J] (32 x |J|), FP64 DMMA.
+// CTA = 4 warps (2 x 2), 64 x 32 tile, warp tile 32 x 16: 53 KB of shared memory and ~110 registers, so
+// that four CTAs share an SM and one CTA's loads / stores overlap the DMMAs of the others.
+// 8-column blocks inside the panel are skipped.
+// ------------------------------------------------------------------------------------------
+constexpr int GU32_BM = 64, GU32_BN = 32, GU32_THREADS = 128, GU32_NB = GU32_BN / 16;
+constexpr int GU32_LDN = G32_B + 4, GU32_LDR = GU32_BN + 2;
+constexpr int GU32_SMEM = (GU32_BM * GU32_LDN + G32_B * GU32_LDR) * (int)sizeof(cplx);
+
+__global__ void __launch_bounds__(GU32_THREADS, 4) gj32_update_kernel(const cplx *__restrict__ Xall, cplx *__restrict__ Yall, long long g_batch,
+                                                                   int n, int k0, const cplx *__restrict__ Mall,
+                                                                   const int *__restrict__ rowAtAll)
+{
+    constexpr int B = G32_B, LDN = GU32_LDN, LDR = GU32_LDR;
+    extern __shared__ __align__(16) unsigned char gu_smem_raw[];
+    cplx *sN = reinterpret_cast<cplx *>(gu_smem_raw);
+    cplx *sR = sN + GU32_BM * LDN;
+
+    const int b = blockIdx.z;
+    const cplx *X = Xall + (long long)b * g_batch;
+    cplx *Y = Yall + (long long)b * g_batch;
+    const cplx *Mult = Mall + (long long)b * n * B;
+    const int *rowAt = rowAtAll + (long long)b * n;
+    const int row0 = blockIdx.y * GU32_BM, col0 = blockIdx.x * GU32_BN;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+
+    for (int e = tid; e < GU32_BM * B; e += GU32_THREADS) {
+        int rr = e / B, k = e % B;
+        bool ok = row0 + rr < n;
+        cp_async16(sN + rr * LDN + k, ok ? Mult + (long long)(row0 + rr) * B + k : Mult, ok ? 16 : 0);
+    }
+    for (int e = tid; e < B * GU32_BN; e += GU32_THREADS) {
+        int k = e / GU32_BN, c = e % GU32_BN;
+        bool ok = col0 + c < n && k0 + k < n;
+        cp_async16(sR + k * LDR + c, ok ? X + (long long)rowAt[k0 + k] * n + col0 + c : X, ok ? 16 : 0);
+    }
+    cp_async_commit();
+
+    constexpr int NB = GU32_NB;
+    const int wr = row0 + (warp >> 1) * 32, wc = col0 + (warp & 1) * (8 * NB);
+    int mb_valid = (n - wr + 7) / 8; mb_valid = mb_valid < 0 ? 0 : (mb_valid > 4 ? 4 : mb_valid);
+    int nb_valid = (n - wc + 7) / 8; nb_valid = nb_valid < 0 ? 0 : (nb_valid > NB ? NB : nb_valid);
+    bool skipj[NB];
+#pragma unroll
+    for (int j = 0; j < NB; j++) { int c = wc + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c < k0 + B); }
+
+    double cre[4][NB][2], cim[4][NB][2];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const int rr = wr + i * 8 + g;
+        const cplx *src = X + (long long)((i < mb_valid && rr < n) ? rowAt[rr] : 0) * n;
+#pragma unroll
+        for (int j = 0; j < NB; j++) {
+            const int c = wc + j * 8 + 2 * t;
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                cplx v = cmake(0.0, 0.0);
+                if (i < mb_valid && !skipj[j] && rr < n && c + q < n) v = src[c + q];
+                cre[i][j][q] = v.x; cim[i][j][q] = v.y;
+            }
+        }
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+    const cplx *cA = sN + (warp >> 1) * 32 * LDN;
+    const cplx *cB = sR + (warp & 1) * (8 * NB);
+#pragma unroll
+    for (int kk = 0; kk < B; kk += 4) {
+        cplx a[4], bb[NB];
+#pragma unroll
+        for (int i = 0; i < 4; i++) a[i] = cA[(i * 8 + g) * LDN + kk + t];
+#pragma unroll
+        for (int j = 0; j < NB; j++) bb[j] = cB[(kk + t) * LDR + j * 8 + g];
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+            if (i < mb_valid) {
+                const double nai = -a[i].y;
+#pragma unroll
+                for (int j = 0; j < NB; j++)
+                    if (!skipj[j]) zmma884(cre[i][j], cim[i][j], a[i].x, a[i].y, nai, bb[j].x, bb[j].y);
+            }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < NB; j++) {
+            const int rr = wr + i * 8 + g, c = wc + j * 8 + 2 * t;
+            if (i < mb_valid && !skipj[j] && rr < n) {
+#pragma unroll
+                for (int q = 0; q < 2; q++)
+                    if (c + q < n) Y[(long long)rr * n + c + q] = cmake(cre[i][j][q], cim[i][j][q]);
+            }
+        }
+}
+
+// out[r][orig[pos]] = X[r][pos]: one warp per row, out of place
+__global__ void gj32_unpermute_kernel(const cplx *__restrict__ Xall, cplx *__restrict__ Yall, long long g_batch, int n,
+                                      const int *__restrict__ origall)
+{
+    const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    const int r = blockIdx.x * nw + warp;
+    if (r >= n) return;
+    const cplx *src = Xall + (long long)b * g_batch + (long long)r * n;
+    cplx *dst = Yall + (long long)b * g_batch + (long long)r * n;
+    const int *orig = origall + (long long)b * n;
+    for (int j = lane; j < n; j += 32) dst[orig[j]] = src[j];
+}
+
+}  // namespace rgf

@@ -19,6 +19,7 @@
 
 #include "../../include/rgf.h"
 #include "gj_inverse.cuh"
+#include "gj_inverse32.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -34,6 +35,17 @@ struct Buf {
 
 }  // namespace
 
+// Per-stream workspace: one cohort of matrices runs all its slices on one stream; cohorts on
+// different streams overlap (the latency-bound panel kernel of one with the DMMA update of another).
+struct Ws {
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    cudaEvent_t done = nullptr;
+    Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
+    size_t upd_used = 0;
+};
+
 struct rgf_plan {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -43,16 +55,15 @@ struct rgf_plan {
     double t = 0.0;
     Buf onsite, bond, hop, bondc;                 // device description
     Buf E, T, status, lead_flags, counters;       // per call
-    Buf G, Nb, Rb, orig, Pa, Pb;                  // sweep workspace (cohort-sized)
+    std::vector<Ws> ws;                           // ws[0] runs on the plan's stream
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
-    Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_T4, l_W;   // decimation workspace
+    Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_T4, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
     int cohort_override = 0;
+    int nstreams = 2;
     int profiling = 0;
     bool in_sweep = false;                        // update-kernel events are taken for the sweep's inverses only
     rgf_stats stats;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
-    size_t upd_used = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     char err[512];
     bool attrs_set = false;
@@ -107,7 +118,8 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<32>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<16>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<8>()));
-    CUDA_TRY(p, cudaFuncSetAttribute(gj_panel2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj_panel2_smem(256)));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     p->attrs_set = true;
     return RGF_OK;
@@ -115,110 +127,140 @@ int set_kernel_attrs(rgf_plan *p)
 
 inline int panel_width(int n) { return n <= 256 ? 32 : (n <= 512 ? 16 : 8); }
 
-int launch_zgemm(rgf_plan *p, const ZgemmArgs &a, int batch)
+int launch_zgemm(rgf_plan *p, cudaStream_t stream, const ZgemmArgs &a, int batch)
 {
     if (a.Mr <= 0 || a.Nc <= 0 || batch <= 0) return RGF_OK;
     dim3 grid((a.Nc + ZG_BN - 1) / ZG_BN, (a.Mr + ZG_BM - 1) / ZG_BM, batch);
-    zgemm_kernel<<<grid, ZG_THREADS, ZG_SMEM, p->stream>>>(a);
+    zgemm_kernel<<<grid, ZG_THREADS, ZG_SMEM, stream>>>(a);
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
     return RGF_OK;
 }
 
-template <int B, int NT>
-void launch_panel(rgf_plan *p, cplx *G, int n, int batch, int k0, cplx *Nb, cplx *Rb, int *orig, int *status)
+int ensure_ws_streams(rgf_plan *p)
 {
-    gj_panel_kernel<B, NT><<<batch, NT, gj_panel_smem<B>(n), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+    if ((int)p->ws.size() == p->nstreams) return RGF_OK;
+    for (size_t i = p->ws.size(); i < (size_t)p->nstreams; i++) {
+        Ws w;
+        if (i == 0) { w.stream = p->stream; }
+        else { CUDA_TRY(p, cudaStreamCreateWithFlags(&w.stream, cudaStreamNonBlocking)); w.own_stream = true; }
+        CUDA_TRY(p, cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
+        p->ws.push_back(w);
+    }
+    return RGF_OK;
 }
 
-template <int B>
-int inverse_impl(rgf_plan *p, cplx *G, int n, int batch, int *status)
+// event pair bracketing one update launch (profiling level 1, sweep only)
+int update_events(rgf_plan *p, Ws &w, cudaEvent_t *e0, cudaEvent_t *e1)
 {
-    cplx *Nb = ptr<cplx>(p->Nb), *Rb = ptr<cplx>(p->Rb);
-    int *orig = ptr<int>(p->orig);
-    int total = n * batch;
-    gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, p->stream>>>(orig, n, total);
-    p->stats.launches++;
-    for (int k0 = 0; k0 < n; k0 += B) {
-        if (B == 32) {
-            gj_panel2_kernel<<<batch, P2_NT, gj_panel2_smem(n), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
-        } else if (B == 16) {
-            launch_panel<16, 512>(p, G, n, batch, k0, Nb, Rb, orig, status);
-        } else {
-            launch_panel<8, 1024>(p, G, n, batch, k0, Nb, Rb, orig, status);
-        }
-        p->stats.launches++;
-        CUDA_TRY(p, cudaGetLastError());
-        if (n > B) {
-            dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
-            bool timed = p->profiling > 0 && p->in_sweep;
-            cudaEvent_t e0 = nullptr, e1 = nullptr;
-            if (timed) {
-                if (p->upd_used == p->upd_events.size()) {
-                    if (p->upd_events.size() >= 2048) {
-                        // drain: accumulate and reuse
-                        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
-                        for (size_t q = 0; q < p->upd_used; q++) {
-                            float ms = 0.f;
-                            cudaEventElapsedTime(&ms, p->upd_events[q].first, p->upd_events[q].second);
-                            p->stats.ms_inverse_update += ms;
-                        }
-                        p->upd_used = 0;
-                    } else {
-                        cudaEvent_t a, b;
-                        CUDA_TRY(p, cudaEventCreate(&a));
-                        CUDA_TRY(p, cudaEventCreate(&b));
-                        p->upd_events.push_back(std::make_pair(a, b));
-                    }
-                }
-                e0 = p->upd_events[p->upd_used].first;
-                e1 = p->upd_events[p->upd_used].second;
-                p->upd_used++;
-                CUDA_TRY(p, cudaEventRecord(e0, p->stream));
+    if (w.upd_used == w.upd_events.size()) {
+        if (w.upd_events.size() >= 2048) {
+            CUDA_TRY(p, cudaStreamSynchronize(w.stream));
+            for (size_t q = 0; q < w.upd_used; q++) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, w.upd_events[q].first, w.upd_events[q].second);
+                p->stats.ms_inverse_update += ms;
             }
-            gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), p->stream>>>(G, (long long)n * n, n, k0, Nb, Rb);
-            if (timed) CUDA_TRY(p, cudaEventRecord(e1, p->stream));
-            p->stats.launches++;
-            if (p->in_sweep) p->stats.launches_inverse_update++;
-            CUDA_TRY(p, cudaGetLastError());
+            w.upd_used = 0;
+        } else {
+            cudaEvent_t a, b;
+            CUDA_TRY(p, cudaEventCreate(&a));
+            CUDA_TRY(p, cudaEventCreate(&b));
+            w.upd_events.push_back(std::make_pair(a, b));
         }
     }
-    int nw = n > 512 ? 4 : 8;
-    dim3 grid((n + nw - 1) / nw, batch);
-    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), p->stream>>>(G, (long long)n * n, n, orig);
-    p->stats.launches++;
-    CUDA_TRY(p, cudaGetLastError());
+    *e0 = w.upd_events[w.upd_used].first;
+    *e1 = w.upd_events[w.upd_used].second;
+    w.upd_used++;
     return RGF_OK;
-}
-
-// workspace for inverting `batch` n x n matrices
-int ensure_inverse_ws(rgf_plan *p, int n, int batch)
-{
-    int B = panel_width(n), rc;
-    if ((rc = ensure(p, p->Nb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
-    if ((rc = ensure(p, p->Rb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
-    if ((rc = ensure(p, p->orig, sizeof(int) * (size_t)n * batch))) return rc;
-    return RGF_OK;
-}
-
-// in-place inverse of `batch` matrices stored at G (stride n*n); status[b] set to 1 on a bad pivot
-int run_inverse(rgf_plan *p, cplx *G, int n, int batch, int *status)
-{
-    if (n > 1024) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 1024 is not supported in this version", n);
-    int B = panel_width(n);
-    if (B == 32) return inverse_impl<32>(p, G, n, batch, status);
-    if (B == 16) return inverse_impl<16>(p, G, n, batch, status);
-    return inverse_impl<8>(p, G, n, batch, status);
 }
 
 void drain_update_events(rgf_plan *p)
 {
-    for (size_t q = 0; q < p->upd_used; q++) {
-        float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, p->upd_events[q].first, p->upd_events[q].second) == cudaSuccess)
-            p->stats.ms_inverse_update += ms;
+    for (Ws &w : p->ws) {
+        for (size_t q = 0; q < w.upd_used; q++) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, w.upd_events[q].first, w.upd_events[q].second) == cudaSuccess)
+                p->stats.ms_inverse_update += ms;
+        }
+        w.upd_used = 0;
     }
-    p->upd_used = 0;
+}
+
+// workspace of stream w for inverting `batch` n x n matrices
+int ensure_inverse_ws(rgf_plan *p, Ws &w, int n, int batch)
+{
+    int B = panel_width(n), rc;
+    if ((rc = ensure(p, w.Nb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
+    if (n > 256 && (rc = ensure(p, w.Rb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
+    if ((rc = ensure(p, w.rowAt, sizeof(int) * (size_t)n * batch))) return rc;
+    if ((rc = ensure(p, w.orig, sizeof(int) * (size_t)n * batch))) return rc;
+    return RGF_OK;
+}
+
+// generic in-place path (256 < n <= 1024): panels of 16 or 8 columns, physical row exchanges
+template <int B, int NT>
+int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status)
+{
+    cplx *Nb = ptr<cplx>(w.Nb), *Rb = ptr<cplx>(w.Rb);
+    int *orig = ptr<int>(w.orig);
+    for (int k0 = 0; k0 < n; k0 += B) {
+        gj_panel_kernel<B, NT><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+        p->stats.launches++;
+        dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
+        gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb);
+        p->stats.launches++;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    int nw = n > 512 ? 4 : 8;
+    dim3 grid((n + nw - 1) / nw, batch);
+    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), w.stream>>>(G, (long long)n * n, n, orig);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    return RGF_OK;
+}
+
+// Inverse of `batch` n x n matrices stored at G (stride n*n).  Galt is a second buffer of the same
+// size; *result is G or Galt, whichever holds the inverse (n <= 256 ping-pongs between the two).
+// status[b] is set to 1 on a zero / non-finite pivot.
+int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, cplx **result)
+{
+    if (n > 1024) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 1024 is not supported in this version", n);
+    int *orig = ptr<int>(w.orig);
+    const int total = n * batch;
+    gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, w.stream>>>(orig, n, total);
+    p->stats.launches++;
+    if (n > 512) { *result = G; return inverse_inplace<8, 1024>(p, w, G, n, batch, status); }
+    if (n > 256) { *result = G; return inverse_inplace<16, 512>(p, w, G, n, batch, status); }
+    cplx *X = G, *Y = Galt, *Mult = ptr<cplx>(w.Nb);
+    int *rowAt = ptr<int>(w.rowAt);
+    const long long gb = (long long)n * n;
+    for (int k0 = 0; k0 < n; k0 += G32_B) {
+        gj32_panel_kernel<<<batch, G32_NT, gj32_panel_smem(n), w.stream>>>(X, Y, gb, n, k0, Mult, rowAt, orig, status);
+        p->stats.launches++;
+        if (n > G32_B) {
+            dim3 grid((n + GU32_BN - 1) / GU32_BN, (n + GU32_BM - 1) / GU32_BM, batch);
+            const bool timed = p->profiling > 0 && p->in_sweep;
+            cudaEvent_t e0 = nullptr, e1 = nullptr;
+            if (timed) {
+                int rc = update_events(p, w, &e0, &e1);
+                if (rc) return rc;
+                CUDA_TRY(p, cudaEventRecord(e0, w.stream));
+            }
+            gj32_update_kernel<<<grid, GU32_THREADS, GU32_SMEM, w.stream>>>(X, Y, gb, n, k0, Mult, rowAt);
+            if (timed) CUDA_TRY(p, cudaEventRecord(e1, w.stream));
+            p->stats.launches++;
+            if (p->in_sweep) p->stats.launches_inverse_update++;
+        }
+        CUDA_TRY(p, cudaGetLastError());
+        std::swap(X, Y);
+    }
+    dim3 grid((n + 7) / 8, batch);
+    gj32_unpermute_kernel<<<grid, 256, 0, w.stream>>>(X, Y, gb, n, orig);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    *result = Y;
+    return RGF_OK;
 }
 
 }  // namespace
@@ -246,7 +288,7 @@ int lead_gemm(rgf_plan *p, const cplx *A, int lda, long long a_batch, const cplx
     a.C = C; a.c_batch = (long long)M * M; a.ldc = M;
     a.Mr = a.Nc = a.K = M;
     a.alpha = cmake(1.0, 0.0);
-    return launch_zgemm(p, a, n_E);
+    return launch_zgemm(p, p->stream, a, n_E);
 }
 
 int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cplx *g_out, int *iters_out, int *n_open_out)
@@ -258,18 +300,19 @@ int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cp
     if ((rc = ensure(p, p->l_eps, sizeof(cplx) * NN * n_E))) return rc;
     if ((rc = ensure(p, p->l_eps_s, sizeof(cplx) * NN * n_E))) return rc;
     if ((rc = ensure(p, p->l_W, sizeof(cplx) * NN * n_E))) return rc;
+    if (N <= 256 && (rc = ensure(p, p->l_W2, sizeof(cplx) * NN * n_E))) return rc;
     Buf *small[] = {&p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4};
     for (Buf *b : small) if ((rc = ensure(p, *b, sizeof(cplx) * MM * n_E))) return rc;
-    if ((rc = ensure_inverse_ws(p, N, n_E))) return rc;
+    Ws &w = p->ws[0];
+    if ((rc = ensure_inverse_ws(p, w, N, n_E))) return rc;
     if ((rc = ensure(p, p->lead_flags, sizeof(int) * (size_t)(n_E + 4)))) return rc;
-    cplx *eps = ptr<cplx>(p->l_eps), *eps_s = ptr<cplx>(p->l_eps_s), *g = ptr<cplx>(p->l_W);
+    cplx *eps = ptr<cplx>(p->l_eps), *eps_s = ptr<cplx>(p->l_eps_s), *gw = ptr<cplx>(p->l_W), *gw2 = ptr<cplx>(p->l_W2), *g = nullptr;
     cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta);
     cplx *T1 = ptr<cplx>(p->l_T1), *X = ptr<cplx>(p->l_T2), *Y = ptr<cplx>(p->l_T3), *T3 = ptr<cplx>(p->l_T4);
     int *flags = ptr<int>(p->lead_flags), *n_open = flags + n_E;
     int *status = ptr<int>(p->status);      // a bad pivot in the lead marks batch items [0, n_E): device 0 of each energy
     const double *E = ptr<double>(p->E);
     dim3 gN((unsigned)std::min<long long>((NN + 255) / 256, 2048), n_E), gM((unsigned)std::min<long long>((MM + 255) / 256, 1024), n_E);
-    const cplx *g11 = g, *g12 = g + M, *g21 = g + (long long)M * N, *g22 = g + (long long)M * N + M;
 
     lead_cell_init_kernel<<<gN, 256, 0, p->stream>>>(eps, eps_s, a, b, M, p->t, pa, pb);
     p->stats.launches++;
@@ -281,9 +324,10 @@ int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cp
         CUDA_TRY(p, cudaMemcpyAsync(&open, n_open, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         if (open == 0) break;
-        lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(g, eps, N, E, eta);
+        lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(gw, eps, N, E, eta);
         p->stats.launches++;
-        if ((rc = run_inverse(p, g, N, n_E, status))) return rc;
+        if ((rc = run_inverse(p, w, gw, gw2, N, n_E, status, &g))) return rc;
+        const cplx *g11 = g, *g12 = g + M, *g21 = g + (long long)M * N, *g22 = g + (long long)M * N + M;
         if ((rc = lead_gemm(p, a, M, MM, g11, N, NN, T1, n_E))) return rc;      // a g11
         if ((rc = lead_gemm(p, T1, M, MM, b, M, MM, X, n_E))) return rc;        // X = a g11 b   -> [2,2]
         if ((rc = lead_gemm(p, b, M, MM, g22, N, NN, T3, n_E))) return rc;      // b g22
@@ -297,9 +341,9 @@ int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cp
         std::swap(a, X);
         std::swap(b, Y);
     }
-    lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(g, eps_s, N, E, eta);
+    lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(gw, eps_s, N, E, eta);
     p->stats.launches++;
-    if ((rc = run_inverse(p, g, N, n_E, status))) return rc;
+    if ((rc = run_inverse(p, w, gw, gw2, N, n_E, status, &g))) return rc;
     lead_extract_kernel<<<gM, 256, 0, p->stream>>>(g, g_out, M, side);
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
@@ -332,37 +376,41 @@ inline const cplx *lead_gR(const rgf_plan *p) { return (p->L & 1) == 0 ? ptr<cpl
 int choose_cohort(const rgf_plan *p, int batch)
 {
     if (p->cohort_override > 0) return std::min(p->cohort_override, batch);
-    return batch;
+    return (batch + p->nstreams - 1) / p->nstreams;      // one cohort per stream
 }
 
-int ensure_sweep_ws(rgf_plan *p, int cohort)
+int ensure_sweep_ws(rgf_plan *p, Ws &w, int cohort)
 {
     int rc;
     const int M = p->M, nh = p->nh;
-    if ((rc = ensure(p, p->G, sizeof(cplx) * (size_t)M * M * cohort))) return rc;
-    if ((rc = ensure(p, p->Pa, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
-    if ((rc = ensure(p, p->Pb, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
-    return ensure_inverse_ws(p, M, cohort);
+    if ((rc = ensure(p, w.G0, sizeof(cplx) * (size_t)M * M * cohort))) return rc;
+    if ((rc = ensure(p, w.G1, sizeof(cplx) * (size_t)M * M * cohort))) return rc;
+    if ((rc = ensure(p, w.Pa, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
+    if ((rc = ensure(p, w.Pb, sizeof(cplx) * (size_t)nh * nh * cohort))) return rc;
+    return ensure_inverse_ws(p, w, M, cohort);
 }
 
-// A3-A5 for the cohort [bz0, bz0+nb): slices 0..nslices-1.  On return G holds g_{nslices-1} and
-// *Pcur the compact propagator.
-int run_sweep_cohort(rgf_plan *p, int n_E, double eta, int bz0, int nb, int nslices, cplx **Pcur_out)
+// A3-A5 for the cohort [bz0, bz0+nb) on workspace w: slices 0..nslices-1.  On return *G_out holds
+// g_{nslices-1}, *Galt_out is the other (free) M x M buffer and *Pcur_out the compact propagator.
+int run_sweep_cohort(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **G_out, cplx **Galt_out,
+                     cplx **Pcur_out)
 {
     const int M = p->M, L = p->L, nh = p->nh;
     int rc;
-    cplx *G = ptr<cplx>(p->G), *Pcur = ptr<cplx>(p->Pa), *Pnext = ptr<cplx>(p->Pb);
+    cplx *G = ptr<cplx>(w.G0), *Galt = ptr<cplx>(w.G1), *Pcur = ptr<cplx>(w.Pa), *Pnext = ptr<cplx>(w.Pb);
     int *status = ptr<int>(p->status) + bz0;
     const double *E = ptr<double>(p->E);
     dim3 ag((unsigned)std::min<long long>(((long long)M * M + 255) / 256, 2048), nb);
     for (int i = 0; i < nslices; i++) {
-        assemble_kernel<<<ag, 256, 0, p->stream>>>(G, M, L, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite),
-                                                  ptr<uint8_t>(p->bond), ptr<uint8_t>(p->hop), ptr<cplx>(p->gL), lead_gR(p));
+        assemble_kernel<<<ag, 256, 0, w.stream>>>(G, M, L, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite),
+                                                 ptr<uint8_t>(p->bond), ptr<uint8_t>(p->hop), ptr<cplx>(p->gL), lead_gR(p));
         p->stats.launches++;
-        if ((rc = run_inverse(p, G, M, nb, status))) return rc;
+        cplx *res = nullptr;
+        if ((rc = run_inverse(p, w, G, Galt, M, nb, status, &res))) return rc;
+        if (res != G) std::swap(G, Galt);
         if (i == 0) {
             dim3 pg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
-            propagator_start_kernel<<<pg, 256, 0, p->stream>>>(G, Pcur, M, nh);
+            propagator_start_kernel<<<pg, 256, 0, w.stream>>>(G, Pcur, M, nh);
             p->stats.launches++;
         } else {
             // P_i[S_i, :] = t * g_i[S_i, S_{i-1}] diag(m'_{i-1}) P_{i-1}[S_{i-1}, :]   (Eq. 5)
@@ -376,26 +424,25 @@ int run_sweep_cohort(rgf_plan *p, int n_E, double eta, int bz0, int nb, int nsli
             a.C = Pnext; a.c_batch = (long long)nh * nh; a.ldc = nh;
             a.Mr = (M - pi + 1) / 2; a.K = (M - pp + 1) / 2; a.Nc = M / 2;
             a.alpha = cmake(p->t, 0.0);
-            if ((rc = launch_zgemm(p, a, nb))) return rc;
+            if ((rc = launch_zgemm(p, w.stream, a, nb))) return rc;
             std::swap(Pcur, Pnext);
         }
     }
     CUDA_TRY(p, cudaGetLastError());
-    *Pcur_out = Pcur;
+    *G_out = G; *Galt_out = Galt; *Pcur_out = Pcur;
     return RGF_OK;
 }
 
 // A6 for the cohort: T = Re Tr[Gamma_L P^dagger Gamma_R P]  (Eq. 2)
-int run_trace_cohort(rgf_plan *p, int n_E, int bz0, int nb, cplx *Pcur)
+int run_trace_cohort(rgf_plan *p, Ws &w, int n_E, int bz0, int nb, cplx *scratch, cplx *Pcur)
 {
     const int M = p->M, L = p->L, nh = p->nh;
     int rc;
-    cplx *scratch = ptr<cplx>(p->G);                   // g_{L-1} is no longer needed
-    cplx *Gam = scratch, *Y = scratch + (size_t)nh * nh * nb;
-    cplx *X = (Pcur == ptr<cplx>(p->Pa)) ? ptr<cplx>(p->Pb) : ptr<cplx>(p->Pa);
+    cplx *Gam = scratch, *Y = scratch + (size_t)nh * nh * nb;      // an M x M buffer per matrix holds both
+    cplx *X = (Pcur == ptr<cplx>(w.Pa)) ? ptr<cplx>(w.Pb) : ptr<cplx>(w.Pa);
     const int pR = (L - 1) & 1, nr = (M - pR + 1) / 2, nc = M / 2;
     dim3 gg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
-    gamma_right_kernel<<<gg, 256, 0, p->stream>>>(Gam, lead_gR(p), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t);
+    gamma_right_kernel<<<gg, 256, 0, w.stream>>>(Gam, lead_gR(p), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t);
     p->stats.launches++;
     ZgemmArgs a;
     memset(&a, 0, sizeof(a));                            // X = Gamma_R P
@@ -403,14 +450,14 @@ int run_trace_cohort(rgf_plan *p, int n_E, int bz0, int nb, cplx *Pcur)
     a.B = Pcur; a.b_batch = (long long)nh * nh; a.ldb = nh;
     a.C = X; a.c_batch = (long long)nh * nh; a.ldc = nh;
     a.Mr = nr; a.K = nr; a.Nc = nc; a.alpha = cmake(1.0, 0.0);
-    if ((rc = launch_zgemm(p, a, nb))) return rc;
+    if ((rc = launch_zgemm(p, w.stream, a, nb))) return rc;
     memset(&a, 0, sizeof(a));                            // Y = P^dagger X
     a.A = Pcur; a.a_batch = (long long)nh * nh; a.a_rs = 1; a.a_cs = nh; a.conjA = 1; a.kmask_div = 1;
     a.B = X; a.b_batch = (long long)nh * nh; a.ldb = nh;
     a.C = Y; a.c_batch = (long long)nh * nh; a.ldc = nh;
     a.Mr = nc; a.K = nr; a.Nc = nc; a.alpha = cmake(1.0, 0.0);
-    if ((rc = launch_zgemm(p, a, nb))) return rc;
-    trace_kernel<<<nb, 256, 0, p->stream>>>(Y, ptr<cplx>(p->gL), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t, ptr<double>(p->T));
+    if ((rc = launch_zgemm(p, w.stream, a, nb))) return rc;
+    trace_kernel<<<nb, 256, 0, w.stream>>>(Y, ptr<cplx>(p->gL), ptr<uint8_t>(p->bond), M, L, nh, n_E, bz0, p->t, ptr<double>(p->T));
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
     return RGF_OK;
@@ -431,6 +478,8 @@ int begin_call(rgf_plan *p)
     if (!p) return RGF_EINVAL;
     p->err[0] = 0;
     CUDA_TRY(p, cudaSetDevice(p->device));
+    int rc = ensure_ws_streams(p);
+    if (rc) return rc;
     return set_kernel_attrs(p);
 }
 
@@ -536,7 +585,7 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
         return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
     }
     memset(&p->stats, 0, sizeof(p->stats));
-    p->upd_used = 0;
+    for (Ws &w : p->ws) w.upd_used = 0;
     CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
     if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
     if ((rc = check_energies_finite(p, n_E))) return rc;
@@ -551,23 +600,28 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     if (rc) return rc;
     p->stats.launches_leads = p->stats.launches;
     CUDA_TRY(p, cudaEventRecord(p->ev[1], p->stream));
+    // ---- sweep + trace: cohorts round-robin over the streams; each cohort is an independent chain
     const int cohort = choose_cohort(p, batch);
     p->stats.cohort = cohort;
-    if ((rc = ensure_sweep_ws(p, cohort))) return rc;
-    float ms_trace = 0.f;
-    for (int bz0 = 0; bz0 < batch; bz0 += cohort) {
+    const int ns = (int)p->ws.size();
+    for (Ws &w : p->ws) if ((rc = ensure_sweep_ws(p, w, cohort))) return rc;
+    for (int i = 1; i < ns; i++) CUDA_TRY(p, cudaStreamWaitEvent(p->ws[i].stream, p->ev[1], 0));
+    nvtxRangePushA("rgf_sweep");
+    p->in_sweep = true;
+    int ci = 0;
+    for (int bz0 = 0; bz0 < batch && rc == RGF_OK; bz0 += cohort, ci++) {
+        Ws &w = p->ws[ci % ns];
         const int nb = std::min(cohort, batch - bz0);
-        cplx *Pcur = nullptr;
-        nvtxRangePushA("rgf_sweep");
-        p->in_sweep = true;
-        rc = run_sweep_cohort(p, n_E, eta, bz0, nb, p->L, &Pcur);
-        p->in_sweep = false;
-        nvtxRangePop();
-        if (rc) return rc;
-        nvtxRangePushA("rgf_trace");
-        rc = run_trace_cohort(p, n_E, bz0, nb, Pcur);
-        nvtxRangePop();
-        if (rc) return rc;
+        cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
+        rc = run_sweep_cohort(p, w, n_E, eta, bz0, nb, p->L, &G, &Galt, &Pcur);
+        if (rc == RGF_OK) rc = run_trace_cohort(p, w, n_E, bz0, nb, Galt, Pcur);
+    }
+    p->in_sweep = false;
+    nvtxRangePop();
+    if (rc) return rc;
+    for (int i = 1; i < ns; i++) {
+        CUDA_TRY(p, cudaEventRecord(p->ws[i].done, p->ws[i].stream));
+        CUDA_TRY(p, cudaStreamWaitEvent(p->stream, p->ws[i].done, 0));
     }
     CUDA_TRY(p, cudaEventRecord(p->ev[2], p->stream));
     // failed energies -> NaN.  Lead failures (flags per energy) hit every device of that energy.
@@ -595,7 +649,7 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     cudaEventElapsedTime(&ms, p->ev[0], p->ev[3]); p->stats.ms_total = ms;
     cudaEventElapsedTime(&ms, p->ev[0], p->ev[1]); p->stats.ms_leads = ms;
     cudaEventElapsedTime(&ms, p->ev[1], p->ev[2]); p->stats.ms_sweep = ms;
-    cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_trace = ms + ms_trace;
+    cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_trace = ms;
     return result;
 }
 
@@ -605,10 +659,17 @@ int rgf_destroy(rgf_plan *p)
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
     Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->counters,
-                   &p->G, &p->Nb, &p->Rb, &p->orig, &p->Pa, &p->Pb, &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha,
-                   &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4, &p->l_W, &p->stage_in, &p->stage_out};
+                   &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4,
+                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out};
     for (Buf *b : bufs) release(*b);
-    for (auto &pr : p->upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+    for (Ws &w : p->ws) {
+        if (w.stream) cudaStreamSynchronize(w.stream);
+        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb};
+        for (Buf *b : wb) release(*b);
+        for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+        if (w.done) cudaEventDestroy(w.done);
+        if (w.own_stream && w.stream) cudaStreamDestroy(w.stream);
+    }
     for (int i = 0; i < 5; i++) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
     delete p;
@@ -688,12 +749,14 @@ int rgf_inverse_batched(rgf_plan *p, int n, int batch, const double *A, double *
     const size_t bytes = sizeof(cplx) * (size_t)n * n * batch;
     if ((rc = ensure(p, p->stage_in, bytes))) return rc;
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
-    if ((rc = ensure_inverse_ws(p, n, batch))) return rc;
+    if ((rc = ensure(p, p->stage_out, bytes))) return rc;
+    if ((rc = ensure_inverse_ws(p, p->ws[0], n, batch))) return rc;
     CUDA_TRY(p, cudaMemcpyAsync(p->stage_in.p, A, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
-    if ((rc = run_inverse(p, ptr<cplx>(p->stage_in), n, batch, ptr<int>(p->status)))) return rc;
+    cplx *res = nullptr;
+    if ((rc = run_inverse(p, p->ws[0], ptr<cplx>(p->stage_in), ptr<cplx>(p->stage_out), n, batch, ptr<int>(p->status), &res))) return rc;
     std::vector<int> h_status(batch);
-    CUDA_TRY(p, cudaMemcpyAsync(Ainv, p->stage_in.p, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(Ainv, res, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     drain_update_events(p);
@@ -754,15 +817,16 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
     if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
-    if ((rc = ensure_sweep_ws(p, n_E))) return rc;
-    cplx *Pcur = nullptr;
-    if ((rc = run_sweep_cohort(p, n_E, eta, dev * n_E, n_E, nslices, &Pcur))) return rc;
+    Ws &w = p->ws[0];
+    if ((rc = ensure_sweep_ws(p, w, n_E))) return rc;
+    cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
+    if ((rc = run_sweep_cohort(p, w, n_E, eta, dev * n_E, n_E, nslices, &G, &Galt, &Pcur))) return rc;
     const size_t bytes = sizeof(cplx) * (size_t)M * M * n_E;
     if ((rc = ensure(p, p->stage_out, bytes))) return rc;
     dim3 grid((unsigned)std::min((M * M + 255) / 256, 2048), n_E);
     propagator_expand_kernel<<<grid, 256, 0, p->stream>>>(Pcur, ptr<cplx>(p->stage_out), M, nh, (nslices - 1) & 1);
     CUDA_TRY(p, cudaGetLastError());
-    CUDA_TRY(p, cudaMemcpyAsync(g_out, p->G.p, bytes, cudaMemcpyDefault, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(g_out, G, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaMemcpyAsync(P_out, p->stage_out.p, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     drain_update_events(p);

@@ -101,3 +101,17 @@ def truncate(w: Workload, L: int, energy_index=None) -> Workload:
     vac = None if w.vacancy is None else np.ascontiguousarray(w.vacancy[:, :L])
     return Workload(w.name + " [first %d slices, %d energies]" % (L, len(E)), w.M, L,
                     np.ascontiguousarray(w.onsite[:, :L]), vac, np.ascontiguousarray(E), w.t, w.eta, dict(w.notes))
+
+
+def shard(energies, world, rank):
+    """Round-robin energy shard of rank `rank` ((seed, energy) pairs are independent)."""
+    return np.ascontiguousarray(np.asarray(energies)[rank::world])
+
+
+def unshard(parts, n_total):
+    """Inverse of shard(): parts[r] holds the results of energies[r::world]."""
+    world = len(parts)
+    out = np.empty((parts[0].shape[0], n_total) if parts[0].ndim == 2 else n_total, dtype=parts[0].dtype)
+    for r, p in enumerate(parts):
+        out[..., r::world] = p
+    return out

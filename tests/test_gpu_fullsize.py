@@ -1,0 +1,84 @@
+"""Full-size parity: the configs of BASELINE.json in the launch configuration bench.py times
+(whole energy batch in one rgf_transmission call), compared on the sampled energies whose oracle
+value is stored under tests/golden/ (written by tests/golden/make_oracle_goldens.py, oracle only),
+plus properties that hold at every energy.  Tolerance: |dT| <= 1e-9 * max(1, T)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1107_5300_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def golden(cfg):
+    g = np.loadtxt(os.path.join(GOLDEN, "config%d_oracle.txt" % cfg))
+    return g[:, 0].astype(int), g[:, 1].astype(int), g[:, 2], g[:, 3]
+
+
+def n_open_channels(M, E, t=-2.7):
+    x = abs(E / t)
+    return sum(1 for p in range(1, M // 2 + 1)
+               if abs(1 - 2 * np.cos(p * np.pi / (M + 1))) < x < 1 + 2 * np.cos(p * np.pi / (M + 1)))
+
+
+def check(w, T, cfg):
+    dev, eidx, E, T_or = golden(cfg)
+    assert np.allclose(w.energies[eidx], E, rtol=0, atol=0)
+    got = T[dev, eidx]
+    err = np.abs(got - T_or) / np.maximum(1.0, np.abs(T_or))
+    assert np.all(err <= 1e-9), (cfg, err.max(), got, T_or)
+    # properties at every energy (Q19): finite, 0 <= T <= number of open lead channels
+    assert np.all(np.isfinite(T))
+    nch = np.array([n_open_channels(w.M, e) for e in w.energies])
+    assert np.all(T >= -1e-9) and np.all(T <= nch[None, :] + 1e-8), (T.min(), (T - nch[None, :]).max())
+    return err.max()
+
+
+@pytest.fixture()
+def plan():
+    from paper_1107_5300_b200 import binding as rgf
+    with rgf.Plan(0) as p:
+        yield p
+
+
+def test_config1_four_seeds_batched(plan):
+    w = inputs.config1()
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)
+    assert T.shape == (4, 256)
+    check(w, T, 1)
+
+
+def test_config2_headline(plan):
+    w = inputs.config2()
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)
+    err = check(w, T, 2)
+    st = plan.stats()
+    print("configs[2]: max rel err %.2e, %.1f s, %d launches" % (err, st["ms_total"] / 1e3, st["launches"]))
+
+
+def test_config3_disordered_c128(plan):
+    w = inputs.config3(disordered=True)
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)
+    check(w, T, 3)
+
+
+def test_config3_clean_c128_closed_form(plan):
+    """configs[3] variant (a): clean M=244, L=2000 against the closed form (skip points within 1e-4 eV of a subband edge, Q8)."""
+    from test_oracle_pins import closed_form_T
+    w = inputs.config3(disordered=False)
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)[0]
+    skipped = 0
+    for e, tk in zip(w.energies, T):
+        Tc, n_open, dist = closed_form_T(w.M, w.L, e, eta=w.eta)
+        if dist < 1e-4:
+            skipped += 1
+            continue
+        assert abs(tk - Tc) < 1e-8 * max(1.0, Tc), (e, tk, Tc)
+    assert skipped <= 16
