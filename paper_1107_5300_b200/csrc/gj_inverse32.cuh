@@ -22,7 +22,7 @@ constexpr int G32_LDP = G32_B + 4;      // 36: A / C fragment accesses conflict-
 constexpr int G32_LDR = G32_B + 2;      // 34
 __host__ __device__ constexpr size_t gj32_panel_smem(int n)
 {
-    return sizeof(cplx) * ((size_t)G32_NT * G32_LDP + G32_SB * G32_LDR + G32_SB) + sizeof(unsigned long long) * 32 +
+    return sizeof(cplx) * ((size_t)G32_NT * G32_LDP + G32_SB * G32_LDR + 2 * (G32_NT / 32) * (G32_SB + 1)) + sizeof(unsigned) * 4 * (G32_NT / 32) +
            sizeof(int) * (2 * (size_t)n + G32_B + 8) + 64;
 }
 
@@ -34,9 +34,11 @@ __global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restri
     extern __shared__ __align__(16) unsigned char gj_smem[];
     cplx *panel = reinterpret_cast<cplx *>(gj_smem);           // [NT][LDP], rows in X order
     cplx *Rs = panel + NT * LDP;                                // [SB][LDR] pivot rows of the sub-block
-    cplx *pivrow = Rs + SB * LDR;                               // [SB]
-    unsigned long long *red = reinterpret_cast<unsigned long long *>(pivrow + SB);   // [32]
-    int *rowAt = reinterpret_cast<int *>(red + 32);
+    cplx *crow = Rs + SB * LDR;                                 // [2][NT/32][SB] candidate pivot rows
+    cplx *cinv = crow + 2 * (NT / 32) * SB;                     // [2][NT/32] 1 / candidate pivot
+    unsigned *ckey = reinterpret_cast<unsigned *>(cinv + 2 * (NT / 32));               // [2][NT/32]
+    int *cidx = reinterpret_cast<int *>(ckey + 2 * (NT / 32));                         // [2][NT/32]
+    int *rowAt = cidx + 2 * (NT / 32);
     int *posOf = rowAt + n;
     int *prow = posOf + n;                                      // [B]
 
@@ -72,45 +74,51 @@ __global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restri
         for (int j = 0; j < SB; j++) row[j] = panel[r * LDP + c0 + j];
 #pragma unroll 1
         for (int cc = 0; cc < ncols; cc++) {
+            const int pb = (cc & 1) * (NT / 32);           // candidate buffers alternate: one barrier per column
             cplx x = row[0];
 #pragma unroll
             for (int j = 1; j < SB; j++) if (j == cc) x = row[j];
-            // ---- pivot search.  Key = (high 32 bits of |x|^2, ~row): the maximum over the block is a
-            // pivot within 2^-20 of the largest magnitude (any such pivot is as good), lowest row on ties.
+            // ---- pivot search.  32-bit key = top 24 bits of |x|^2 (sign, exponent, 12 mantissa bits) and
+            // 255 - warp: the block maximum is a pivot within 2^-12 of the largest magnitude (any such
+            // pivot is as good as the exact maximum), lowest warp / lowest lane on ties.  Each warp's
+            // candidate lane publishes its raw row, its row index and 1/x, so one barrier per column suffices.
             const double v = cabs2(x);
-            unsigned hi = used ? 0u : (unsigned)__double2hiint(v);
+            unsigned hi = used ? 0u : ((unsigned)__double2hiint(v) & 0xffffff00u);
             if (!used && !(v == v)) hi = 0x7ff80000u;                 // NaN: report it
             const unsigned wmax = __reduce_max_sync(0xffffffffu, hi);
             const unsigned ball = __ballot_sync(0xffffffffu, hi == wmax);
-            if (lane == 0) red[warp] = ((unsigned long long)wmax << 32) | (unsigned)(0xffffffffu - (unsigned)(warp * 32 + __ffs(ball) - 1));
-            __syncthreads();
-            unsigned long long best = red[0];
-#pragma unroll
-            for (int w = 1; w < NT / 32; w++) { unsigned long long o = red[w]; best = o > best ? o : best; }
-            const int pr = (int)(0xffffffffu - (unsigned)(best & 0xffffffffu));
-            if (r == pr) {
-                const unsigned bh = (unsigned)(best >> 32);
-                if (bh == 0u || bh >= 0x7ff00000u) status[b] = 1;     // zero / non-finite pivot
+            if (lane == __ffs(ball) - 1) {
+                ckey[pb + warp] = wmax | (unsigned)(255 - warp);
+                cidx[pb + warp] = r;
                 const double iv = 1.0 / v;                             // 1/x = conj(x) / |x|^2
-                const cplx d = cmake(x.x * iv, -x.y * iv);
+                cinv[pb + warp] = cmake(x.x * iv, -x.y * iv);
 #pragma unroll
-                for (int j = 0; j < SB; j++) {
-                    cplx y = (j == cc) ? cmake(1.0, 0.0) : row[j];
-                    row[j] = cmul(y, d);
-                    pivrow[j] = row[j];
-                }
+                for (int j = 0; j < SB; j++) crow[(pb + warp) * SB + j] = row[j];
+            }
+            __syncthreads();
+            unsigned best = ckey[pb];
+#pragma unroll
+            for (int w = 1; w < NT / 32; w++) best = max(best, ckey[pb + w]);
+            const int pw = 255 - (int)(best & 0xffu);
+            const int pr = cidx[pb + pw];
+            const cplx d = cinv[pb + pw];
+            if (r == pr) {
+                if ((best >> 8) == 0u || best >= 0x7ff00000u) status[b] = 1;     // zero / non-finite pivot
+#pragma unroll
+                for (int j = 0; j < SB; j++) row[j] = (j == cc) ? d : cmul(row[j], d);
                 used = true;
                 const int k = k0 + c0 + cc, a = rowAt[k], pp = posOf[pr];
                 rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
                 prow[c0 + cc] = pr;
-            }
-            __syncthreads();
-            if (r != pr) {
+            } else {
+                // row -= (x / x_piv) * pivot row; the pivot column itself becomes -x / x_piv
+                const cplx f = cmul(x, d);
 #pragma unroll
                 for (int j = 0; j < SB; j++) {
-                    cplx y = (j == cc) ? cmake(0.0, 0.0) : row[j];
-                    cfnma(y, x, pivrow[j]);
-                    row[j] = y;
+                    const cplx pj = crow[(pb + pw) * SB + j];
+                    cplx y = row[j];
+                    cfnma(y, f, pj);
+                    row[j] = (j == cc) ? cmake(-f.x, -f.y) : y;
                 }
             }
         }
@@ -204,16 +212,26 @@ __global__ void __launch_bounds__(GU32_THREADS, 4) gj32_update_kernel(const cplx
     const int *rowAt = rowAtAll + (long long)b * n;
     const int row0 = blockIdx.y * GU32_BM, col0 = blockIdx.x * GU32_BN;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    // tile entirely inside the panel: nothing to do (a predicated-off DMMA still occupies the tensor pipe)
+    if (col0 >= k0 && col0 + GU32_BN <= k0 + B) return;
 
-    for (int e = tid; e < GU32_BM * B; e += GU32_THREADS) {
-        int rr = e / B, k = e % B;
+    // the row maps this tile needs, fetched once (dependent global loads would otherwise serialise
+    // every copy below behind a rowAt lookup)
+    __shared__ int sRowK[G32_B], sRowM[GU32_BM];
+    if (tid < G32_B) sRowK[tid] = (k0 + tid < n) ? rowAt[k0 + tid] : 0;
+    else if (tid < G32_B + GU32_BM) { int rr = row0 + tid - G32_B; sRowM[tid - G32_B] = rr < n ? rowAt[rr] : 0; }
+#pragma unroll
+    for (int it = 0; it < (GU32_BM * B) / GU32_THREADS; it++) {
+        int e = tid + it * GU32_THREADS, rr = e / B, k = e % B;
         bool ok = row0 + rr < n;
         cp_async16(sN + rr * LDN + k, ok ? Mult + (long long)(row0 + rr) * B + k : Mult, ok ? 16 : 0);
     }
-    for (int e = tid; e < B * GU32_BN; e += GU32_THREADS) {
-        int k = e / GU32_BN, c = e % GU32_BN;
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < (B * GU32_BN) / GU32_THREADS; it++) {
+        int e = tid + it * GU32_THREADS, k = e / GU32_BN, c = e % GU32_BN;
         bool ok = col0 + c < n && k0 + k < n;
-        cp_async16(sR + k * LDR + c, ok ? X + (long long)rowAt[k0 + k] * n + col0 + c : X, ok ? 16 : 0);
+        cp_async16(sR + k * LDR + c, ok ? X + (long long)sRowK[k] * n + col0 + c : X, ok ? 16 : 0);
     }
     cp_async_commit();
 
@@ -229,7 +247,7 @@ __global__ void __launch_bounds__(GU32_THREADS, 4) gj32_update_kernel(const cplx
 #pragma unroll
     for (int i = 0; i < 4; i++) {
         const int rr = wr + i * 8 + g;
-        const cplx *src = X + (long long)((i < mb_valid && rr < n) ? rowAt[rr] : 0) * n;
+        const cplx *src = X + (long long)((i < mb_valid && rr < n) ? sRowM[rr - row0] : 0) * n;
 #pragma unroll
         for (int j = 0; j < NB; j++) {
             const int c = wc + j * 8 + 2 * t;

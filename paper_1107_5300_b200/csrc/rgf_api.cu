@@ -60,7 +60,7 @@ struct rgf_plan {
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_T4, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
     int cohort_override = 0;
-    int nstreams = 2;
+    int nstreams = 1;
     int profiling = 0;
     bool in_sweep = false;                        // update-kernel events are taken for the sweep's inverses only
     rgf_stats stats;

@@ -31,6 +31,7 @@ constexpr int ZG_BM = 64, ZG_BN = 64, ZG_BK = 16, ZG_THREADS = 128;
 constexpr int ZG_LDA = ZG_BK + 4;    // 20
 constexpr int ZG_LDB = ZG_BN + 2;    // 66
 constexpr int ZG_STAGES = 2;
+constexpr int ZG_KMASK_MAX = 1024;     // masked GEMMs have K <= ceil(M/2) <= 512
 constexpr int ZG_SMEM = ZG_STAGES * (ZG_BM * ZG_LDA + ZG_BK * ZG_LDB) * (int)sizeof(cplx);
 
 // One k4 step of a warp tile of MB x NB DMMA blocks.  sA points at the warp's first row,
@@ -71,6 +72,13 @@ __global__ void __launch_bounds__(ZG_THREADS) zgemm_kernel(ZgemmArgs p)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
     const bool k_fast = p.a_cs <= p.a_rs;
+    // k mask staged once: a global byte load in front of every copy would serialise the stage loads
+    __shared__ uint8_t sKmask[ZG_KMASK_MAX];
+    const bool masked = kmask != nullptr;
+    if (masked) {
+        for (int k = tid; k < p.K && k < ZG_KMASK_MAX; k += ZG_THREADS) sKmask[k] = kmask[k];
+        __syncthreads();
+    }
 
     auto load_stage = [&](int stage, int k0) {
         cplx *dA = sA + stage * ZG_BM * ZG_LDA;
@@ -80,7 +88,7 @@ __global__ void __launch_bounds__(ZG_THREADS) zgemm_kernel(ZgemmArgs p)
             int idx = tid + e * ZG_THREADS, r, k;
             if (k_fast) { r = idx / ZG_BK; k = idx % ZG_BK; } else { k = idx / ZG_BM; r = idx % ZG_BM; }
             int gr = row0 + r, gk = k0 + k;
-            bool ok = gr < p.Mr && gk < p.K && (!kmask || kmask[gk]);
+            bool ok = gr < p.Mr && gk < p.K && (!masked || sKmask[gk]);
             const cplx *src = ok ? A + (long long)gr * p.a_rs + (long long)gk * p.a_cs : A;
             cp_async16(dA + r * ZG_LDA + k, src, ok ? 16 : 0);
         }
