@@ -24,7 +24,7 @@
 namespace rgf {
 
 // ------------------------------------------------------------------------------------------
-// Panel factorisation.  blockDim.x = NT >= n (one thread per row).  Dynamic shared memory:
+// Panel factorisation.  blockDim.x = NT, NT * ROWS >= n (thread tid owns rows tid + q NT).  Dynamic shared memory:
 //   pivrow[B] cplx | red_val[32] double | red_idx[32] int | rowAt[n] int | posOf[n] int |
 //   moved[2B] int | nmoved | stage[2B][GJ_CH] cplx
 // ------------------------------------------------------------------------------------------
@@ -37,7 +37,7 @@ __host__ __device__ constexpr size_t gj_panel_smem(int n)
            sizeof(int) * (2 * B + 4) + sizeof(cplx) * 2 * B * GJ_CH + 64;
 }
 
-template <int B, int NT>
+template <int B, int NT, int ROWS>
 __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_batch, int n, int k0,
                                                       cplx *Nall, cplx *Rall, int *origall, int *status)
 {
@@ -57,30 +57,38 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     cplx *Rbuf = Rall + (long long)b * n * B;
     int *orig = origall + (long long)b * n;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int r = tid;
-    const bool has_row = r < n;
     const int bw = (n - k0 < B) ? (n - k0) : B;
 
-    cplx row[B];
+    // thread tid owns rows tid, tid + NT, ... (ROWS of them), each with its B panel entries in registers
+    cplx row[ROWS][B];
+    bool used[ROWS];
 #pragma unroll
-    for (int c = 0; c < B; c++) row[c] = (has_row && c < bw) ? G[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
+    for (int q = 0; q < ROWS; q++) {
+        const int r = tid + q * NT;
+#pragma unroll
+        for (int c = 0; c < B; c++) row[q][c] = (r < n && c < bw) ? G[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
+        used[q] = (r >= n || r < k0);     // positions < k0 hold the pivot rows of earlier panels
+    }
     for (int i = tid; i < n; i += NT) { rowAt[i] = i; posOf[i] = i; }
-    bool used = !has_row || r < k0 ? true : false;   // rows above the panel were pivots of earlier panels
-    // NOTE: rows at positions < k0 are the pivot rows of previous panels (exchanges were made
-    // physical), so the search set is positions >= k0.
     __syncthreads();
 
     // The column loop is a real loop (an unrolled one is ~400 KB of straight-line code and runs at
     // instruction-fetch speed); the register-resident row is indexed with select chains instead.
 #pragma unroll 1
     for (int c = 0; c < bw; c++) {
-        cplx x = row[0];
+        cplx x[ROWS];
+        double v = -1.0;
+        int idx = tid;
 #pragma unroll
-        for (int j = 1; j < B; j++) if (j == c) x = row[j];
-        // ---- pivot search: max |x|^2 over unused rows, lowest row index on ties
-        double v = used ? -1.0 : cabs2(x);
-        if (!(v == v)) v = 1e300;                 // NaN: make it win so that it is reported
-        int idx = r;
+        for (int q = 0; q < ROWS; q++) {
+            x[q] = row[q][0];
+#pragma unroll
+            for (int j = 1; j < B; j++) if (j == c) x[q] = row[q][j];
+            // ---- pivot search: max |x|^2 over unused rows, lowest row index on ties
+            double vq = used[q] ? -1.0 : cabs2(x[q]);
+            if (!(vq == vq)) vq = 1e300;          // NaN: make it win so that it is reported
+            if (vq > v) { v = vq; idx = tid + q * NT; }
+        }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             double ov = __shfl_xor_sync(0xffffffffu, v, off);
@@ -95,27 +103,33 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
             double ov = red_val[w]; int oi = red_idx[w];
             if (ov > bv || (ov == bv && oi < pr)) { bv = ov; pr = oi; }
         }
-        if (r == pr) {
-            if (!(bv > 0.0) || !(bv < 1e299)) status[b] = 1;          // zero / non-finite pivot
-            cplx d = crecip(x);
 #pragma unroll
-            for (int j = 0; j < B; j++) {
-                cplx y = (j == c) ? cmake(1.0, 0.0) : row[j];
-                row[j] = cmul(y, d);
-                pivrow[j] = row[j];
+        for (int q = 0; q < ROWS; q++) {
+            if (tid + q * NT == pr) {
+                if (!(bv > 0.0) || !(bv < 1e299)) status[b] = 1;          // zero / non-finite pivot
+                cplx d = crecip(x[q]);
+#pragma unroll
+                for (int j = 0; j < B; j++) {
+                    cplx y = (j == c) ? cmake(1.0, 0.0) : row[q][j];
+                    row[q][j] = cmul(y, d);
+                    pivrow[j] = row[q][j];
+                }
+                used[q] = true;
+                // exchange positions k (= k0 + c) and the position currently holding row pr
+                int k = k0 + c, a = rowAt[k], pp = posOf[pr];
+                rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
             }
-            used = true;
-            // exchange positions k (= k0 + c) and the position currently holding row pr
-            int k = k0 + c, a = rowAt[k], pp = posOf[pr];
-            rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
         }
         __syncthreads();
-        if (has_row && r != pr) {
 #pragma unroll
-            for (int j = 0; j < B; j++) {
-                cplx y = (j == c) ? cmake(0.0, 0.0) : row[j];
-                cfnma(y, x, pivrow[j]);
-                row[j] = y;
+        for (int q = 0; q < ROWS; q++) {
+            if (tid + q * NT < n && tid + q * NT != pr) {
+#pragma unroll
+                for (int j = 0; j < B; j++) {
+                    cplx y = (j == c) ? cmake(0.0, 0.0) : row[q][j];
+                    cfnma(y, x[q], pivrow[j]);
+                    row[q][j] = y;
+                }
             }
         }
         // pivrow / red_* are rewritten only after the next column's first barrier
@@ -131,14 +145,18 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     const int nm = *nmoved;                      // <= 2B
 
     // ---- new panel columns and multipliers (row r now lives at position posOf[r])
-    if (has_row) {
-        const int pos = posOf[r];
 #pragma unroll
-        for (int c = 0; c < B; c++) {
-            if (c < bw) G[(long long)pos * n + k0 + c] = row[c];
-            cplx m = row[c];
-            if (pos == k0 + c) m.x -= 1.0;
-            Nbuf[(long long)pos * B + c] = (c < bw) ? m : cmake(0.0, 0.0);
+    for (int q = 0; q < ROWS; q++) {
+        const int r = tid + q * NT;
+        if (r < n) {
+            const int pos = posOf[r];
+#pragma unroll
+            for (int c = 0; c < B; c++) {
+                if (c < bw) G[(long long)pos * n + k0 + c] = row[q][c];
+                cplx m = row[q][c];
+                if (pos == k0 + c) m.x -= 1.0;
+                Nbuf[(long long)pos * B + c] = (c < bw) ? m : cmake(0.0, 0.0);
+            }
         }
     }
     // ---- origin bookkeeping: orig[pos] <- orig[rowAt[pos]]
@@ -195,6 +213,7 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     // whole tile inside the panel: nothing to do
     if (col0 >= k0 && col0 + GU_BN <= k0 + B) return;
+    static_assert(B % 4 == 0, "panel width must be a multiple of the DMMA k");
 
     for (int e = tid; e < GU_BM * B; e += GU_THREADS) {
         int rr = e / B, k = e % B;
@@ -213,7 +232,7 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
     int nb_valid = (n - col0 + 7) / 8; nb_valid = nb_valid > 4 ? 4 : nb_valid;
     bool skipj[4];
 #pragma unroll
-    for (int j = 0; j < 4; j++) { int c = col0 + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c < k0 + B); }
+    for (int j = 0; j < 4; j++) { int c = col0 + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c + 8 <= k0 + B); }
 
     double cre[4][4][2], cim[4][4][2];
 #pragma unroll
@@ -255,7 +274,8 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
             if (i < mb_valid && !skipj[j] && rr < n) {
 #pragma unroll
                 for (int q = 0; q < 2; q++)
-                    if (c + q < n) G[(long long)rr * n + c + q] = cmake(cre[i][j][q], cim[i][j][q]);
+                    if (c + q < n && !(c + q >= k0 && c + q < k0 + B))      // panel columns hold N' already
+                        G[(long long)rr * n + c + q] = cmake(cre[i][j][q], cim[i][j][q]);
             }
         }
 }

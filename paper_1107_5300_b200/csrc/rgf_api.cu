@@ -118,6 +118,7 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<32>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<16>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<8>()));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<4>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
@@ -125,7 +126,7 @@ int set_kernel_attrs(rgf_plan *p)
     return RGF_OK;
 }
 
-inline int panel_width(int n) { return n <= 256 ? 32 : (n <= 512 ? 16 : 8); }
+inline int panel_width(int n) { return n <= 256 ? 32 : (n <= 512 ? 16 : (n <= 1024 ? 8 : 4)); }
 
 int launch_zgemm(rgf_plan *p, cudaStream_t stream, const ZgemmArgs &a, int batch)
 {
@@ -199,13 +200,13 @@ int ensure_inverse_ws(rgf_plan *p, Ws &w, int n, int batch)
 }
 
 // generic in-place path (256 < n <= 1024): panels of 16 or 8 columns, physical row exchanges
-template <int B, int NT>
+template <int B, int NT, int ROWS>
 int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status)
 {
     cplx *Nb = ptr<cplx>(w.Nb), *Rb = ptr<cplx>(w.Rb);
     int *orig = ptr<int>(w.orig);
     for (int k0 = 0; k0 < n; k0 += B) {
-        gj_panel_kernel<B, NT><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
         p->stats.launches++;
         dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
         gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb);
@@ -225,13 +226,14 @@ int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status)
 // status[b] is set to 1 on a zero / non-finite pivot.
 int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, cplx **result)
 {
-    if (n > 1024) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 1024 is not supported in this version", n);
+    if (n > 2048) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 2048 is not supported in this version", n);
     int *orig = ptr<int>(w.orig);
     const int total = n * batch;
     gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, w.stream>>>(orig, n, total);
     p->stats.launches++;
-    if (n > 512) { *result = G; return inverse_inplace<8, 1024>(p, w, G, n, batch, status); }
-    if (n > 256) { *result = G; return inverse_inplace<16, 512>(p, w, G, n, batch, status); }
+    if (n > 1024) { *result = G; return inverse_inplace<4, 1024, 2>(p, w, G, n, batch, status); }
+    if (n > 512) { *result = G; return inverse_inplace<8, 1024, 1>(p, w, G, n, batch, status); }
+    if (n > 256) { *result = G; return inverse_inplace<16, 512, 1>(p, w, G, n, batch, status); }
     cplx *X = G, *Y = Galt, *Mult = ptr<cplx>(w.Nb);
     int *rowAt = ptr<int>(w.rowAt);
     const long long gb = (long long)n * n;
@@ -294,7 +296,7 @@ int lead_gemm(rgf_plan *p, const cplx *A, int lda, long long a_batch, const cplx
 int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cplx *g_out, int *iters_out, int *n_open_out)
 {
     const int M = p->M, N = 2 * M;
-    if (N > 1024) return fail(p, RGF_EUNSUPPORTED, "lead decimation needs a %d x %d inverse; M > 512 is not supported in this version", N, N);
+    if (N > 2048) return fail(p, RGF_EUNSUPPORTED, "lead decimation needs a %d x %d inverse; M > 1024 is not supported in this version", N, N);
     const long long MM = (long long)M * M, NN = (long long)N * N;
     int rc;
     if ((rc = ensure(p, p->l_eps, sizeof(cplx) * NN * n_E))) return rc;

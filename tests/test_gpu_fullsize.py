@@ -82,3 +82,18 @@ def test_config3_clean_c128_closed_form(plan):
             continue
         assert abs(tk - Tc) < 1e-8 * max(1.0, Tc), (e, tk, Tc)
     assert skipped <= 16
+
+
+def test_config4_wide_ribbon_truncated(plan):
+    """configs[4] (M = 1024, edge vacancies): the first 24 slices of the same arrays, leads attached at
+    slice 24 (the naive oracle needs hours per energy at full length), 4 energies."""
+    path = os.path.join(GOLDEN, "config4_oracle.txt")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/config4_oracle.txt not generated yet")
+    dev, eidx, E, T_or = golden(4)
+    w = inputs.truncate(inputs.config4(), 24, eidx)
+    assert np.array_equal(w.energies, E)
+    plan.set_device(w.onsite, w.t, w.vacancy)
+    T = plan.transmission(w.energies, w.eta)[0]
+    err = np.abs(T - T_or) / np.maximum(1.0, np.abs(T_or))
+    assert np.all(err <= 1e-9), (err.max(), T, T_or)
