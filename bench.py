@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--L", type=int, default=8000)
     ap.add_argument("--n-E", type=int, default=512)
     ap.add_argument("--cohort", type=int, default=0)
+    ap.add_argument("--form", default="half", choices=["half", "dense"], help="formulation of the sweep (include/rgf.h)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -184,6 +185,7 @@ def main():
     plan = rgf.rgf_plan_create(local, stream.cuda_stream)
     if a.cohort:
         rgf.rgf_set_cohort(plan, a.cohort)
+    rgf.rgf_set_formulation(plan, rgf.RGF_FORM_HALF if a.form == "half" else rgf.RGF_FORM_DENSE)
     peak = rgf.rgf_fp64_peak_tflops(plan)
     rgf.rgf_set_device(plan, w.M, w.L, onsite, w.t, None)
     E_dev = torch.from_numpy(E_host).to(dev)
@@ -243,17 +245,21 @@ def main():
     units_step = world * n_E * w.L                        # slice-steps per step over all ranks
     if rank == 0:
         value = units_step * a.steps / (ms_max * 1e-3)
-        fl_inv, l_inv = update_flops_per_inverse(w.M)
+        n_inv = w.M // 2 if a.form == "half" else w.M          # matrix size of the inverses (M even at the headline)
+        fl_inv, l_inv = update_flops_per_inverse(n_inv)
         flops_per_launch = fl_inv / max(l_inv, 1) * stats["cohort"]
         avg_ms = ms_upd / max(n_upd, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) * 1e-12 if avg_ms > 0 else 0.0
-        flops_step = n_E * w.L * (8.0 * w.M ** 3 + 8.0 * (w.M / 2) ** 3)      # executed: dense inverse + compact propagator
+        if a.form == "half":
+            flops_step = n_E * w.L * 2 * (8.0 * n_inv ** 3 + 8.0 * n_inv ** 3)     # executed: 2 x ((M/2) inverse + (M/2)^3 GEMM)
+        else:
+            flops_step = n_E * w.L * (8.0 * w.M ** 3 + 8.0 * (w.M / 2) ** 3)      # executed: dense inverse + compact propagator
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[2] armchair ribbon M=%d L=%d n_E=%d per GPU, Anderson +-0.1 eV seed 5300, complex128" % (w.M, w.L, n_E),
-                       "eta": w.eta, "t": w.t, "cohort": stats["cohort"],
+                       "eta": w.eta, "t": w.t, "cohort": stats["cohort"], "formulation": a.form,
                        "l2_policy": "inputs larger than L2 (%.0f MB of state per step)" % (stats["cohort"] * w.M * w.M * 16 / 1e6)},
             "energies_per_s": world * n_E * a.steps / (ms_max * 1e-3),
             "tflops_executed": flops_step * world * a.steps / (ms_max * 1e-3) * 1e-12,

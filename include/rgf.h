@@ -104,6 +104,17 @@ int rgf_get_stats(const rgf_plan *p, rgf_stats *out);
  * launch with events (adds a little launch overhead; used by bench.py for the roofline line). */
 int rgf_set_profiling(rgf_plan *p, int level);
 
+/* Formulation of the sweep.  Both are the recursion of PAPER.md:47-51 (Eq. 4-5) and give the same T(E):
+ *   RGF_FORM_DENSE  one step per slice: complex M x M inverse + compact propagator GEMM, as
+ *                   BASELINE.json:north_star words it (8 M^3 + M^3 real flops per slice-step);
+ *   RGF_FORM_HALF   (default) the same recursion on the finer slicing B_0, F_0, B_1, F_1, ... where
+ *                   F_i / B_i are the atoms of slice i bonded forwards / backwards (the armchair
+ *                   inter-slice coupling t*diag(mask) touches only one of them): two steps per slice,
+ *                   each a complex (M/2) x (M/2) inverse + (M/2)^3 GEMM (4 M^3 real flops per slice-step).
+ * In RGF_FORM_HALF rgf_sweep_state returns only the F_i x F_i block of G_ii (NaN elsewhere). */
+enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1 };
+int rgf_set_formulation(rgf_plan *p, int formulation);
+
 /* Matrices per kernel launch in the sweep (0 = library default = the whole batch).  The sweep runs
  * cohort after cohort over all slices; a cohort whose state fits the 126 MB L2 keeps it there. */
 int rgf_set_cohort(rgf_plan *p, int cohort);

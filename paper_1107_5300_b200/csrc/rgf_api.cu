@@ -20,6 +20,7 @@
 #include "../../include/rgf.h"
 #include "gj_inverse.cuh"
 #include "gj_inverse32.cuh"
+#include "half_kernels.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -42,6 +43,7 @@ struct Ws {
     bool own_stream = false;
     cudaEvent_t done = nullptr;
     Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
+    Buf H0, H1, H2, Wc, Tr;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
     size_t upd_used = 0;
 };
@@ -62,6 +64,7 @@ struct rgf_plan {
     int cohort_override = 0;
     int nstreams = 1;
     int profiling = 0;
+    int formulation = RGF_FORM_HALF;
     bool in_sweep = false;                        // update-kernel events are taken for the sweep's inverses only
     rgf_stats stats;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -201,21 +204,21 @@ int ensure_inverse_ws(rgf_plan *p, Ws &w, int n, int batch)
 
 // generic in-place path (256 < n <= 1024): panels of 16 or 8 columns, physical row exchanges
 template <int B, int NT, int ROWS>
-int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status)
+int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status, long long gb)
 {
     cplx *Nb = ptr<cplx>(w.Nb), *Rb = ptr<cplx>(w.Rb);
     int *orig = ptr<int>(w.orig);
     for (int k0 = 0; k0 < n; k0 += B) {
-        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb, orig, status);
+        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, gb, n, k0, Nb, Rb, orig, status);
         p->stats.launches++;
         dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
-        gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, (long long)n * n, n, k0, Nb, Rb);
+        gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, gb, n, k0, Nb, Rb);
         p->stats.launches++;
         CUDA_TRY(p, cudaGetLastError());
     }
     int nw = n > 512 ? 4 : 8;
     dim3 grid((n + nw - 1) / nw, batch);
-    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), w.stream>>>(G, (long long)n * n, n, orig);
+    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), w.stream>>>(G, gb, n, orig);
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
     return RGF_OK;
@@ -224,19 +227,19 @@ int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status)
 // Inverse of `batch` n x n matrices stored at G (stride n*n).  Galt is a second buffer of the same
 // size; *result is G or Galt, whichever holds the inverse (n <= 256 ping-pongs between the two).
 // status[b] is set to 1 on a zero / non-finite pivot.
-int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, cplx **result)
+int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, cplx **result, long long stride = 0)
 {
+    const long long gb = stride > 0 ? stride : (long long)n * n;
     if (n > 2048) return fail(p, RGF_EUNSUPPORTED, "matrix size %d > 2048 is not supported in this version", n);
     int *orig = ptr<int>(w.orig);
     const int total = n * batch;
     gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, w.stream>>>(orig, n, total);
     p->stats.launches++;
-    if (n > 1024) { *result = G; return inverse_inplace<4, 1024, 2>(p, w, G, n, batch, status); }
-    if (n > 512) { *result = G; return inverse_inplace<8, 1024, 1>(p, w, G, n, batch, status); }
-    if (n > 256) { *result = G; return inverse_inplace<16, 512, 1>(p, w, G, n, batch, status); }
+    if (n > 1024) { *result = G; return inverse_inplace<4, 1024, 2>(p, w, G, n, batch, status, gb); }
+    if (n > 512) { *result = G; return inverse_inplace<8, 1024, 1>(p, w, G, n, batch, status, gb); }
+    if (n > 256) { *result = G; return inverse_inplace<16, 512, 1>(p, w, G, n, batch, status, gb); }
     cplx *X = G, *Y = Galt, *Mult = ptr<cplx>(w.Nb);
     int *rowAt = ptr<int>(w.rowAt);
-    const long long gb = (long long)n * n;
     for (int k0 = 0; k0 < n; k0 += G32_B) {
         gj32_panel_kernel<<<batch, G32_NT, gj32_panel_smem(n), w.stream>>>(X, Y, gb, n, k0, Mult, rowAt, orig, status);
         p->stats.launches++;
@@ -435,6 +438,72 @@ int run_sweep_cohort(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, i
     return RGF_OK;
 }
 
+// ---- half-slice formulation (half_kernels.cuh): 2 half-steps per slice, each an (M/2) inverse and an (M/2)^3 GEMM ----
+int ensure_sweep_ws_half(rgf_plan *p, Ws &w, int cohort)
+{
+    int rc;
+    const int nh = p->nh;
+    const size_t hb = sizeof(cplx) * (size_t)nh * nh * cohort;
+    Buf *bufs[] = {&w.H0, &w.H1, &w.H2, &w.Wc, &w.Pa, &w.Pb};
+    for (Buf *b : bufs) if ((rc = ensure(p, *b, hb))) return rc;
+    if ((rc = ensure(p, w.Tr, 2 * hb))) return rc;
+    return ensure_inverse_ws(p, w, nh, cohort);
+}
+
+// slices 0..nslices-1 of the cohort [bz0, bz0+nb); *g_out = gF of the last slice (dense n x n at stride nh*nh),
+// *Pcur_out its compact propagator (rows F_i, columns B_0, ld nh)
+int run_sweep_cohort_half(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
+{
+    const int M = p->M, L = p->L, nh = p->nh, nc = M / 2;
+    const long long hs = (long long)nh * nh;
+    int rc;
+    cplx *gprev = ptr<cplx>(w.H0), *fa = ptr<cplx>(w.H1), *fb = ptr<cplx>(w.H2);
+    cplx *Pcur = ptr<cplx>(w.Pa), *Pnext = ptr<cplx>(w.Pb), *W = ptr<cplx>(w.Wc);
+    int *status = ptr<int>(p->status) + bz0;
+    HalfArgs ha;
+    memset(&ha, 0, sizeof(ha));
+    ha.M = M; ha.L = L; ha.nh = nh; ha.n_E = n_E; ha.bz0 = bz0; ha.eta = eta; ha.t = p->t;
+    ha.energies = ptr<double>(p->E); ha.onsite = ptr<double>(p->onsite);
+    ha.bond = ptr<uint8_t>(p->bond); ha.hop = ptr<uint8_t>(p->hop);
+    ha.gL = ptr<cplx>(p->gL); ha.gR = lead_gR(p);
+    dim3 eg((unsigned)std::min((int)((hs + 255) / 256), 1024), nb);
+    for (int i = 0; i < nslices; i++) {
+        for (int kind = 0; kind < 2; kind++) {
+            const int par = kind == 0 ? ((i + 1) & 1) : (i & 1);
+            const int n = half_count(M, par);
+            ha.i = i; ha.kind = kind;
+            if (n == 0) continue;           // M = 1 is rejected earlier; n >= 1 always for M >= 2
+            half_assemble_kernel<<<eg, 256, 0, w.stream>>>(fa, gprev, ha);
+            p->stats.launches++;
+            cplx *res = nullptr;
+            if ((rc = run_inverse(p, w, fa, fb, n, nb, status, &res, hs))) return rc;
+            // rotate: res becomes gprev, the other two are free
+            cplx *other = (res == fa) ? fb : fa;
+            cplx *old = gprev;
+            gprev = res; fa = old; fb = other;
+            if (i == 0 && kind == 0) {
+                half_start_kernel<<<eg, 256, 0, w.stream>>>(Pcur, gprev, n, nh);
+                p->stats.launches++;
+            } else {
+                half_couple_kernel<<<eg, 256, 0, w.stream>>>(W, Pcur, ha);
+                p->stats.launches++;
+                ZgemmArgs a;
+                memset(&a, 0, sizeof(a));
+                a.A = gprev; a.a_batch = hs; a.a_rs = n; a.a_cs = 1; a.kmask_div = 1;
+                a.B = W; a.b_batch = hs; a.ldb = nh;
+                a.C = Pnext; a.c_batch = hs; a.ldc = nh;
+                a.Mr = n; a.K = n; a.Nc = nc;
+                a.alpha = cmake(1.0, 0.0);
+                if ((rc = launch_zgemm(p, w.stream, a, nb))) return rc;
+                std::swap(Pcur, Pnext);
+            }
+        }
+    }
+    CUDA_TRY(p, cudaGetLastError());
+    *g_out = gprev; *Pcur_out = Pcur;
+    return RGF_OK;
+}
+
 // A6 for the cohort: T = Re Tr[Gamma_L P^dagger Gamma_R P]  (Eq. 2)
 int run_trace_cohort(rgf_plan *p, Ws &w, int n_E, int bz0, int nb, cplx *scratch, cplx *Pcur)
 {
@@ -606,7 +675,8 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     const int cohort = choose_cohort(p, batch);
     p->stats.cohort = cohort;
     const int ns = (int)p->ws.size();
-    for (Ws &w : p->ws) if ((rc = ensure_sweep_ws(p, w, cohort))) return rc;
+    const bool half = p->formulation == RGF_FORM_HALF;
+    for (Ws &w : p->ws) if ((rc = half ? ensure_sweep_ws_half(p, w, cohort) : ensure_sweep_ws(p, w, cohort))) return rc;
     for (int i = 1; i < ns; i++) CUDA_TRY(p, cudaStreamWaitEvent(p->ws[i].stream, p->ev[1], 0));
     nvtxRangePushA("rgf_sweep");
     p->in_sweep = true;
@@ -615,7 +685,12 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
         Ws &w = p->ws[ci % ns];
         const int nb = std::min(cohort, batch - bz0);
         cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
-        rc = run_sweep_cohort(p, w, n_E, eta, bz0, nb, p->L, &G, &Galt, &Pcur);
+        if (half) {
+            rc = run_sweep_cohort_half(p, w, n_E, eta, bz0, nb, p->L, &G, &Pcur);
+            Galt = ptr<cplx>(w.Tr);
+        } else {
+            rc = run_sweep_cohort(p, w, n_E, eta, bz0, nb, p->L, &G, &Galt, &Pcur);
+        }
         if (rc == RGF_OK) rc = run_trace_cohort(p, w, n_E, bz0, nb, Galt, Pcur);
     }
     p->in_sweep = false;
@@ -666,7 +741,7 @@ int rgf_destroy(rgf_plan *p)
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
-        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb};
+        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
         if (w.done) cudaEventDestroy(w.done);
@@ -691,6 +766,13 @@ int rgf_set_profiling(rgf_plan *p, int level)
 {
     if (!p || level < 0 || level > 1) return RGF_EINVAL;
     p->profiling = level;
+    return RGF_OK;
+}
+
+int rgf_set_formulation(rgf_plan *p, int formulation)
+{
+    if (!p || (formulation != RGF_FORM_DENSE && formulation != RGF_FORM_HALF)) return RGF_EINVAL;
+    p->formulation = formulation;
     return RGF_OK;
 }
 
@@ -820,12 +902,20 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
     if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
     Ws &w = p->ws[0];
-    if ((rc = ensure_sweep_ws(p, w, n_E))) return rc;
+    const bool half = p->formulation == RGF_FORM_HALF;
+    if ((rc = half ? ensure_sweep_ws_half(p, w, n_E) : ensure_sweep_ws(p, w, n_E))) return rc;
     cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
-    if ((rc = run_sweep_cohort(p, w, n_E, eta, dev * n_E, n_E, nslices, &G, &Galt, &Pcur))) return rc;
     const size_t bytes = sizeof(cplx) * (size_t)M * M * n_E;
     if ((rc = ensure(p, p->stage_out, bytes))) return rc;
     dim3 grid((unsigned)std::min((M * M + 255) / 256, 2048), n_E);
+    if (half) {
+        if ((rc = run_sweep_cohort_half(p, w, n_E, eta, dev * n_E, n_E, nslices, &G, &Pcur))) return rc;
+        if ((rc = ensure(p, p->stage_in, bytes))) return rc;
+        half_expand_g_kernel<<<grid, 256, 0, p->stream>>>(G, ptr<cplx>(p->stage_in), M, nh, (nslices - 1) & 1);
+        G = ptr<cplx>(p->stage_in);
+    } else {
+        if ((rc = run_sweep_cohort(p, w, n_E, eta, dev * n_E, n_E, nslices, &G, &Galt, &Pcur))) return rc;
+    }
     propagator_expand_kernel<<<grid, 256, 0, p->stream>>>(Pcur, ptr<cplx>(p->stage_out), M, nh, (nslices - 1) & 1);
     CUDA_TRY(p, cudaGetLastError());
     CUDA_TRY(p, cudaMemcpyAsync(g_out, G, bytes, cudaMemcpyDefault, p->stream));

@@ -25,6 +25,18 @@ def plan(rgf):
         yield p
 
 
+FORMS = [0, 1]          # RGF_FORM_DENSE, RGF_FORM_HALF (include/rgf.h)
+
+
+@pytest.fixture(params=FORMS, ids=["dense", "half"])
+def fplan(rgf, request):
+    """A plan in each formulation of the sweep."""
+    with rgf.Plan(0) as p:
+        rgf.rgf_set_formulation(p.handle, request.param)
+        p.form = request.param
+        yield p
+
+
 def tol(T):
     return 1e-9 * np.maximum(1.0, np.abs(T))
 
@@ -96,7 +108,8 @@ def test_lead_self_energy_matches_oracle(rgf, plan, oracle, M, L):
 # ---- A3-A5: state of the sweep ---------------------------------------------------------------
 
 @pytest.mark.parametrize("M,L,ns", [(20, 12, 1), (20, 12, 2), (20, 12, 7), (21, 9, 9), (64, 6, 5)])
-def test_sweep_state_matches_oracle(rgf, plan, oracle, M, L, ns):
+def test_sweep_state_matches_oracle(rgf, fplan, oracle, M, L, ns):
+    plan = fplan
     on = inputs.anderson(M, L, 0.25, 99 + M)
     plan.set_device(on, -2.7)
     E = np.array([-1.1, 0.07, 0.9])
@@ -105,7 +118,13 @@ def test_sweep_state_matches_oracle(rgf, plan, oracle, M, L, ns):
     rgf.rgf_sweep_state(plan.handle, 0, E, 3, 1e-9, rgf.RGF_C128, ns, g, P)
     for k, e in enumerate(E):
         g0, P0 = oracle.sweep_state(on, None, -2.7, e, 1e-9, ns)
-        assert np.max(np.abs(g[k] - g0)) < 1e-9 * np.max(np.abs(g0))
+        if plan.form == rgf.RGF_FORM_HALF:       # only the F_i x F_i block of G_ii exists in this formulation
+            hg = ~np.isnan(g[k].real)
+            fr = (np.arange(M) % 2) == ((ns - 1) % 2)
+            assert np.array_equal(hg, np.outer(fr, fr))
+            assert np.max(np.abs(g[k][hg] - g0[hg])) < 1e-9 * np.max(np.abs(g0))
+        else:
+            assert np.max(np.abs(g[k] - g0)) < 1e-9 * np.max(np.abs(g0))
         have = ~np.isnan(P[k].real)
         rows = (np.arange(M) % 2) == ((ns - 1) % 2)
         cols = (np.arange(M) % 2) == 1
@@ -115,7 +134,8 @@ def test_sweep_state_matches_oracle(rgf, plan, oracle, M, L, ns):
 
 # ---- end to end ----------------------------------------------------------------------------
 
-def test_config0_matches_oracle_and_closed_form(rgf, plan, oracle):
+def test_config0_matches_oracle_and_closed_form(rgf, fplan, oracle):
+    plan = fplan
     from test_oracle_pins import closed_form_T
     w = inputs.config0()
     plan.set_device(w.onsite, w.t)
@@ -127,8 +147,9 @@ def test_config0_matches_oracle_and_closed_form(rgf, plan, oracle):
     assert plan.stats()["launches"] > 0
 
 
-@pytest.mark.parametrize("M,L,W", [(20, 1, 0.2), (20, 2, 0.2), (21, 17, 0.3), (50, 33, 0.25), (128, 24, 0.25)])
-def test_disordered_small_matches_oracle(rgf, plan, oracle, M, L, W):
+@pytest.mark.parametrize("M,L,W", [(2, 3, 0.2), (3, 4, 0.2), (20, 1, 0.2), (20, 2, 0.2), (21, 17, 0.3), (50, 33, 0.25), (128, 24, 0.25)])
+def test_disordered_small_matches_oracle(rgf, fplan, oracle, M, L, W):
+    plan = fplan
     on = inputs.anderson(M, L, W, 1000 + M + L)
     E = np.linspace(-1.0, 1.0, 8)
     plan.set_device(on, -2.7)
@@ -137,7 +158,8 @@ def test_disordered_small_matches_oracle(rgf, plan, oracle, M, L, W):
     assert np.all(np.abs(T - T_or) <= tol(T_or)), np.max(np.abs(T - T_or))
 
 
-def test_batched_devices_vacancies_and_cohorts(rgf, plan, oracle):
+def test_batched_devices_vacancies_and_cohorts(rgf, fplan, oracle):
+    plan = fplan
     """4 devices batched (configs[1] shape, reduced), one with edge vacancies; ragged cohorts."""
     M, L = 32, 20
     on = np.stack([inputs.anderson(M, L, 0.25, s) for s in (1107, 1108, 1109)])
