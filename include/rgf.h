@@ -111,8 +111,13 @@ int rgf_set_profiling(rgf_plan *p, int level);
  *                   F_i / B_i are the atoms of slice i bonded forwards / backwards (the armchair
  *                   inter-slice coupling t*diag(mask) touches only one of them): two steps per slice,
  *                   each a complex (M/2) x (M/2) inverse + (M/2)^3 GEMM (4 M^3 real flops per slice-step).
- * In RGF_FORM_HALF rgf_sweep_state returns only the F_i x F_i block of G_ii (NaN elsewhere). */
-enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1 };
+ *                   For M <= 256 the whole sweep of one (device, energy) pair is ONE fused kernel
+ *                   (one CTA per pair; inverse and propagator product are a single Gauss-Jordan
+ *                   elimination on [A | C P]); larger M runs it operation by operation;
+ *   RGF_FORM_HALF_STEPWISE  the half-slice recursion launched operation by operation for every M
+ *                   (what RGF_FORM_HALF does for M > 256; exported so that it is testable at small M).
+ * In the half-slice formulations rgf_sweep_state returns only the F_i x F_i block of G_ii (NaN elsewhere). */
+enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1, RGF_FORM_HALF_STEPWISE = 2 };
 int rgf_set_formulation(rgf_plan *p, int formulation);
 
 /* Matrices per kernel launch in the sweep (0 = library default = the whole batch).  The sweep runs

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librgf_b200.so")
 
 RGF_C128, RGF_C64 = 0, 1
-RGF_FORM_DENSE, RGF_FORM_HALF = 0, 1
+RGF_FORM_DENSE, RGF_FORM_HALF, RGF_FORM_HALF_STEPWISE = 0, 1, 2
 RGF_OK, RGF_EINVAL, RGF_ECUDA, RGF_ENOMEM, RGF_ENOCONV, RGF_ESINGULAR, RGF_ESTATE, RGF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7
 
 if not os.path.exists(LIB_PATH):

@@ -21,6 +21,7 @@
 #include "gj_inverse.cuh"
 #include "gj_inverse32.cuh"
 #include "half_kernels.cuh"
+#include "half_sweep.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -43,7 +44,7 @@ struct Ws {
     bool own_stream = false;
     cudaEvent_t done = nullptr;
     Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
-    Buf H0, H1, H2, Wc, Tr;                        // half-slice formulation: three compact g buffers, C P, trace scratch
+    Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
     size_t upd_used = 0;
 };
@@ -124,6 +125,7 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<4>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
+    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     p->attrs_set = true;
     return RGF_OK;
@@ -452,8 +454,53 @@ int ensure_sweep_ws_half(rgf_plan *p, Ws &w, int cohort)
 
 // slices 0..nslices-1 of the cohort [bz0, bz0+nb); *g_out = gF of the last slice (dense n x n at stride nh*nh),
 // *Pcur_out its compact propagator (rows F_i, columns B_0, ld nh)
+inline bool use_fused(const rgf_plan *p) { return p->formulation == RGF_FORM_HALF && p->nh <= HS_NMAX; }
+
+// fused path (half_sweep.cuh): one CTA per matrix runs every half-step of slices 0..nslices-1 in ONE launch
+int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
+{
+    const int nh = p->nh, ldn = (nh + 1) & ~1;
+    int rc;
+    const size_t xb = sizeof(cplx) * (size_t)ldn * ldn * nb;
+    Buf *bufs[] = {&w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1};
+    for (Buf *b : bufs) if ((rc = ensure(p, *b, xb))) return rc;
+    if ((rc = ensure(p, w.Fperm, sizeof(int) * (size_t)HS_NMAX * nb))) return rc;
+    HSweepArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = p->M; a.L = p->L; a.nh = nh; a.ldn = ldn; a.n_E = n_E; a.bz0 = bz0; a.nb = nb; a.eta = eta; a.t = p->t;
+    a.energies = ptr<double>(p->E); a.onsite = ptr<double>(p->onsite);
+    a.bond = ptr<uint8_t>(p->bond); a.hop = ptr<uint8_t>(p->hop);
+    a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
+    a.X0 = ptr<cplx>(w.Fx0); a.X1 = ptr<cplx>(w.Fx1); a.P0 = ptr<cplx>(w.Fp0); a.P1 = ptr<cplx>(w.Fp1);
+    a.perm = ptr<int>(w.Fperm); a.status = ptr<int>(p->status) + bz0;
+    a.hs_begin = 0; a.hs_end = 2 * nslices;
+    a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
+    static const bool prof_on = getenv("RGF_HS_PROF") != nullptr;          // debugging aid: per-phase cycle counters
+    if (prof_on) {
+        if ((rc = ensure(p, p->counters, sizeof(long long) * 8 * (size_t)nb))) return rc;
+        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * 8 * (size_t)nb, w.stream));
+        a.prof = ptr<long long>(p->counters);
+    }
+    half_sweep_kernel<<<nb, HS_NT, sizeof(HSmem), w.stream>>>(a);
+    if (prof_on) {
+        std::vector<long long> h(8 * (size_t)nb);
+        CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->counters.p, sizeof(long long) * h.size(), cudaMemcpyDeviceToHost, w.stream));
+        CUDA_TRY(p, cudaStreamSynchronize(w.stream));
+        double s[8] = {0};
+        for (int b = 0; b < nb; b++) for (int k = 0; k < 8; k++) s[k] += (double)h[8 * (size_t)b + k];
+        const double hsn = (double)nb * a.hs_end;
+        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f\n",
+                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn);
+    }
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    *g_out = ptr<cplx>(w.H0); *Pcur_out = ptr<cplx>(w.Pa);
+    return RGF_OK;
+}
+
 int run_sweep_cohort_half(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
 {
+    if (use_fused(p)) return run_sweep_cohort_fused(p, w, n_E, eta, bz0, nb, nslices, g_out, Pcur_out);
     const int M = p->M, L = p->L, nh = p->nh, nc = M / 2;
     const long long hs = (long long)nh * nh;
     int rc;
@@ -675,7 +722,7 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     const int cohort = choose_cohort(p, batch);
     p->stats.cohort = cohort;
     const int ns = (int)p->ws.size();
-    const bool half = p->formulation == RGF_FORM_HALF;
+    const bool half = p->formulation != RGF_FORM_DENSE;
     for (Ws &w : p->ws) if ((rc = half ? ensure_sweep_ws_half(p, w, cohort) : ensure_sweep_ws(p, w, cohort))) return rc;
     for (int i = 1; i < ns; i++) CUDA_TRY(p, cudaStreamWaitEvent(p->ws[i].stream, p->ev[1], 0));
     nvtxRangePushA("rgf_sweep");
@@ -741,7 +788,7 @@ int rgf_destroy(rgf_plan *p)
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
-        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr};
+        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
         if (w.done) cudaEventDestroy(w.done);
@@ -771,7 +818,7 @@ int rgf_set_profiling(rgf_plan *p, int level)
 
 int rgf_set_formulation(rgf_plan *p, int formulation)
 {
-    if (!p || (formulation != RGF_FORM_DENSE && formulation != RGF_FORM_HALF)) return RGF_EINVAL;
+    if (!p || formulation < RGF_FORM_DENSE || formulation > RGF_FORM_HALF_STEPWISE) return RGF_EINVAL;
     p->formulation = formulation;
     return RGF_OK;
 }
@@ -902,7 +949,7 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
     if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
     Ws &w = p->ws[0];
-    const bool half = p->formulation == RGF_FORM_HALF;
+    const bool half = p->formulation != RGF_FORM_DENSE;
     if ((rc = half ? ensure_sweep_ws_half(p, w, n_E) : ensure_sweep_ws(p, w, n_E))) return rc;
     cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
     const size_t bytes = sizeof(cplx) * (size_t)M * M * n_E;

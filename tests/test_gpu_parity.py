@@ -25,10 +25,10 @@ def plan(rgf):
         yield p
 
 
-FORMS = [0, 1]          # RGF_FORM_DENSE, RGF_FORM_HALF (include/rgf.h)
+FORMS = [0, 1, 2]          # RGF_FORM_DENSE, RGF_FORM_HALF (fused kernel for M <= 256), RGF_FORM_HALF_STEPWISE (include/rgf.h)
 
 
-@pytest.fixture(params=FORMS, ids=["dense", "half"])
+@pytest.fixture(params=FORMS, ids=["dense", "half", "half_stepwise"])
 def fplan(rgf, request):
     """A plan in each formulation of the sweep."""
     with rgf.Plan(0) as p:
@@ -118,7 +118,7 @@ def test_sweep_state_matches_oracle(rgf, fplan, oracle, M, L, ns):
     rgf.rgf_sweep_state(plan.handle, 0, E, 3, 1e-9, rgf.RGF_C128, ns, g, P)
     for k, e in enumerate(E):
         g0, P0 = oracle.sweep_state(on, None, -2.7, e, 1e-9, ns)
-        if plan.form == rgf.RGF_FORM_HALF:       # only the F_i x F_i block of G_ii exists in this formulation
+        if plan.form != rgf.RGF_FORM_DENSE:       # only the F_i x F_i block of G_ii exists in this formulation
             hg = ~np.isnan(g[k].real)
             fr = (np.arange(M) % 2) == ((ns - 1) % 2)
             assert np.array_equal(hg, np.outer(fr, fr))
