@@ -37,8 +37,10 @@ struct HSweepArgs {
     cplx *X0, *X1, *P0, *P1;      // [nb][ldn*ldn] each
     int *perm;                    // [nb][HS_NMAX]
     int *status;                  // [nb]
-    int hs_begin, hs_end;         // half-steps [begin, end): hs = 2 i + kind
-    long long *prof;              // optional [nb][8] cycle counters of thread 0 per phase (NULL = off)
+    int hs_begin, hs_end;         // half-steps [begin, end) of the whole sweep: hs = 2 i + kind
+    int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
+                                  // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
+    long long *prof;              // optional [nb][16] cycle counters of thread 0 per phase (NULL = off)
     cplx *g_out, *P_out;          // after half-step hs_end - 1: g dense n x n (ld n) and P (ld nh), stride nh*nh; may be NULL
 };
 
@@ -47,11 +49,11 @@ struct HSmem {
     cplx R[2][HS_B * HS_LDR];
     cplx crow[2 * (HS_NT / 32) * HS_SB];
     cplx cinv[2 * (HS_NT / 32)];
-    unsigned ckey[2 * (HS_NT / 32)];
-    int cidx[2 * (HS_NT / 32)];
+    alignas(16) unsigned ckey[2 * (HS_NT / 32)];
     int perm[HS_NMAX], pinv[HS_NMAX], perm_prev[HS_NMAX], pinv_prev[HS_NMAX];
     int prow[HS_B];
     int flag;
+    long long prof[16];          // per-phase cycle counters of thread 0 (debugging aid, RGF_HS_PROF)
 };
 
 // per-row tables of the assembly; aliases HSmem::crow while no panel is being factored
@@ -67,75 +69,119 @@ __device__ __forceinline__ cplx ldcg(const cplx *p)
     return v;
 }
 
-// 1 / v for v = |x|^2 > 0: single-precision seed + two Newton steps in FP64 (4 dependent DFMAs instead of
-// the ~30 of the IEEE division, which sits on the critical path of every pivot); falls back to the division
-// outside the float range.  Relative error ~1e-16, irrelevant for a pivot reciprocal.
+// 32-byte (two complex128) L2 load / store: LDG.E.256 / STG.E.256 on sm_100a; p must be 32-byte aligned
+__device__ __forceinline__ void ld256cg(const cplx *p, double &a, double &b, double &c, double &d)
+{
+    asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+__device__ __forceinline__ void st256(cplx *p, double a, double b, double c, double d)
+{
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
+// 1 / v for v = |x|^2 > 0 on the critical path of every pivot: MUFU.RCP64H seed (20 bits) + two Newton steps
+// (4 dependent DFMAs, ~60 cycles) instead of the IEEE division (~130 cycles on sm_100a).  Relative error
+// ~2e-16, irrelevant for a pivot reciprocal.  v outside the normal range (|x| < 1e-154 or > 1e154) gives 0 / inf /
+// NaN, which the caller reports as a singular pivot through the key check and the propagated non-finite values.
 __device__ __forceinline__ double hs_rcp(double v)
 {
-    if (!(v > 1e-30 && v < 1e30)) return 1.0 / v;
-    double r = (double)__frcp_rn((float)v);
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));
     double e = fma(-v, r, 1.0);
     r = fma(r, e, r);
     e = fma(-v, r, 1.0);
-    return fma(r, e, r);
+    r = fma(r, e, r);
+    return r;
 }
+
+#ifdef HS_DBG
+__device__ long long hs_dbg[8];
+#endif
 
 // barrier among the first nthreads threads of the CTA (whole warps); id 1 (0 is __syncthreads)
 __device__ __forceinline__ void hs_bar_active(int nthreads) { asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory"); }
 
-// one pivot step on column CC (static) of the thread's 8-column sub-block
+// One pivot step on column CC (static) of the thread's 8-column sub-block.  Candidate buffers alternate with
+// the parity of CC, so one barrier per column suffices.  32-bit key = top 24 bits of |x|^2 (sign, exponent,
+// 12 mantissa bits: any pivot within 2^-12 of the largest magnitude is as good as the maximum) and 255 - row,
+// so the key is unique, names the row, and the lowest row wins ties.  The pivot row is not a divergent branch:
+//   row[j] <- c + a * pivrow[j]   with (a, c) = (d, 0) on the pivot row and (-x d, row[j]) elsewhere, row[CC] <- a.
 template <int CC>
-__device__ __forceinline__ void hs_pivot_step(HSmem &sm, cplx (&row)[HS_SB], bool &used, int r, int lane, int warp, int naw,
+__device__ __forceinline__ void hs_pivot_step(HSmem &sm, cplx (&row)[HS_SB], bool &used, int r, int warp, int naw,
                                               int kglob, int *status_slot)
 {
     constexpr int SB = HS_SB, NW = HS_NT / 32;
     constexpr int pb = (CC & 1) * NW;
+#ifdef HS_DBG
+    long long td0 = clock64();
+#define HS_DBGT(k) do { long long n_ = clock64(); if (threadIdx.x == 0) hs_dbg[k] += n_ - td0; td0 = n_; } while (0)
+#else
+#define HS_DBGT(k)
+#endif
     const cplx x = row[CC];
-    // 32-bit key: top 24 bits of |x|^2 and 255 - warp (lowest warp / lane wins ties)
-    const double v = cabs2(x);
-    unsigned hi = used ? 0u : ((unsigned)__double2hiint(v) & 0xffffff00u);
-    if (!used && !(v == v)) hi = 0x7ff80000u;
-    const unsigned wmax = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned ball = __ballot_sync(0xffffffffu, hi == wmax);
-    if (lane == __ffs(ball) - 1) {
-        sm.ckey[pb + warp] = wmax | (unsigned)(255 - warp);
-        sm.cidx[pb + warp] = r;
+    // search key from max(|re|, |im|) (integer compare of the high words: no FP64 op on the critical path; the
+    // chosen pivot is within sqrt(2) * (1 + 2^-12) of the largest modulus, as good for partial pivoting)
+    const unsigned hre = (unsigned)__double2hiint(x.x) & 0x7fffffffu, him = (unsigned)__double2hiint(x.y) & 0x7fffffffu;
+    const unsigned hi = used ? 0u : (max(hre, him) & 0xffffff00u);
+    const unsigned key = hi | (unsigned)(255 - r);
+    const double v = cabs2(x);                    // for the reciprocal; overlaps the warp reduction
+    const unsigned wmax = __reduce_max_sync(0xffffffffu, key);
+    HS_DBGT(0);
+    if (key == wmax) {
+        sm.ckey[pb + warp] = key;
         const double iv = hs_rcp(v);
         sm.cinv[pb + warp] = cmake(x.x * iv, -x.y * iv);
 #pragma unroll
-        for (int j = 0; j < SB; j++) sm.crow[(pb + warp) * SB + j] = row[j];
+        for (int j = 0; j < SB; j++) if (j != CC) sm.crow[(pb + warp) * SB + j] = row[j];
     }
+    HS_DBGT(1);
     hs_bar_active(naw * 32);
-    unsigned best = sm.ckey[pb];
-#pragma unroll
-    for (int w = 1; w < NW; w++) if (w < naw) best = max(best, sm.ckey[pb + w]);
-    const int pw = 255 - (int)(best & 0xffu);
-    const int pr = sm.cidx[pb + pw];
+    HS_DBGT(2);
+    const uint4 k4 = *reinterpret_cast<const uint4 *>(&sm.ckey[pb]);
+    unsigned best = k4.x;
+    if (naw > 1) best = max(best, k4.y);
+    if (naw > 2) best = max(best, k4.z);
+    if (naw > 3) best = max(best, k4.w);
+    if (naw > 4) {
+        const uint4 k5 = *reinterpret_cast<const uint4 *>(&sm.ckey[pb + 4]);
+        best = max(best, k5.x);
+        if (naw > 5) best = max(best, k5.y);
+        if (naw > 6) best = max(best, k5.z);
+        if (naw > 7) best = max(best, k5.w);
+    }
+    const int pr = 255 - (int)(best & 0xffu), pw = pr >> 5;
+    HS_DBGT(3);
     const cplx d = sm.cinv[pb + pw];
-    if (r == pr) {
-        if ((best >> 8) == 0u || best >= 0x7ff00000u) *status_slot = 1;
+    const bool is_piv = (r == pr);
+    const cplx nf = cmake(fma(-x.x, d.x, x.y * d.y), fma(-x.x, d.y, -x.y * d.x));     // -(x d)
+    const cplx a = is_piv ? d : nf;
 #pragma unroll
-        for (int j = 0; j < SB; j++) row[j] = (j == CC) ? d : cmul(row[j], d);
+    for (int j = 0; j < SB; j++) {
+        if (j == CC) { row[j] = a; continue; }
+        const cplx pj = sm.crow[(pb + pw) * SB + j];
+        cplx c = is_piv ? cmake(0.0, 0.0) : row[j];
+        c.x = fma(a.x, pj.x, c.x); c.x = fma(-a.y, pj.y, c.x);
+        c.y = fma(a.x, pj.y, c.y); c.y = fma(a.y, pj.x, c.y);
+        row[j] = c;
+    }
+    HS_DBGT(4);
+    if (is_piv) {
+        if ((best >> 8) == 0u || best >= 0x7ff00000u) *status_slot = 1;
         used = true;
         sm.prow[kglob & (HS_B - 1)] = pr;
         sm.perm[kglob] = pr;
         sm.pinv[pr] = kglob;
-    } else {
-        const cplx f = cmul(x, d);
-#pragma unroll
-        for (int j = 0; j < SB; j++) {
-            const cplx pj = sm.crow[(pb + pw) * SB + j];
-            if (j == CC) row[j] = cmake(-f.x, -f.y);
-            else cfnma(row[j], f, pj);
-        }
     }
+    HS_DBGT(5);
+#undef HS_DBGT
 }
 
 // ---- panel factorisation in shared memory: columns [k0, k0 + bw) of all n rows --------------------
 // On entry sm.panel[r][c] = X[r][k0 + c] (zero for c >= bw, r >= n).  On exit sm.panel = N' (the
 // transformed columns), sm.prow[c] = pivot row of column k0 + c, perm / pinv updated, used |= pivot.
-__device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw, bool &used, int *status_slot)
+__device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw, bool &used, int *status_slot, long long *prof)
 {
+    long long tp = prof ? clock64() : 0;
     constexpr int B = HS_B, SB = HS_SB, NT = HS_NT, LDP = HS_LDP, LDR = HS_LDR;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const int r = tid;
@@ -147,6 +193,7 @@ __device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw
         const int c0 = s * SB;
         const int ncols = bw - c0 < SB ? bw - c0 : SB;
         if (ncols <= 0) break;
+        if (prof) tp = clock64();
         cplx row[SB];
         if (has_row) {
 #pragma unroll
@@ -157,16 +204,17 @@ __device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw
         }
         if (warp < naw) {
             const int kg = k0 + c0;
-            hs_pivot_step<0>(sm, row, used, r, lane, warp, naw, kg, status_slot);
-            if (ncols > 1) hs_pivot_step<1>(sm, row, used, r, lane, warp, naw, kg + 1, status_slot);
-            if (ncols > 2) hs_pivot_step<2>(sm, row, used, r, lane, warp, naw, kg + 2, status_slot);
-            if (ncols > 3) hs_pivot_step<3>(sm, row, used, r, lane, warp, naw, kg + 3, status_slot);
-            if (ncols > 4) hs_pivot_step<4>(sm, row, used, r, lane, warp, naw, kg + 4, status_slot);
-            if (ncols > 5) hs_pivot_step<5>(sm, row, used, r, lane, warp, naw, kg + 5, status_slot);
-            if (ncols > 6) hs_pivot_step<6>(sm, row, used, r, lane, warp, naw, kg + 6, status_slot);
-            if (ncols > 7) hs_pivot_step<7>(sm, row, used, r, lane, warp, naw, kg + 7, status_slot);
+            hs_pivot_step<0>(sm, row, used, r, warp, naw, kg, status_slot);
+            if (ncols > 1) hs_pivot_step<1>(sm, row, used, r, warp, naw, kg + 1, status_slot);
+            if (ncols > 2) hs_pivot_step<2>(sm, row, used, r, warp, naw, kg + 2, status_slot);
+            if (ncols > 3) hs_pivot_step<3>(sm, row, used, r, warp, naw, kg + 3, status_slot);
+            if (ncols > 4) hs_pivot_step<4>(sm, row, used, r, warp, naw, kg + 4, status_slot);
+            if (ncols > 5) hs_pivot_step<5>(sm, row, used, r, warp, naw, kg + 5, status_slot);
+            if (ncols > 6) hs_pivot_step<6>(sm, row, used, r, warp, naw, kg + 6, status_slot);
+            if (ncols > 7) hs_pivot_step<7>(sm, row, used, r, warp, naw, kg + 7, status_slot);
         }
         __syncthreads();
+        if (prof) { long long now_ = clock64(); if (tid == 0) sm.prof[5] += now_ - tp; tp = now_; }
         if (has_row) {
 #pragma unroll
             for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
@@ -236,53 +284,62 @@ __device__ __forceinline__ void hs_stage_R(HSmem &sm, int buf, const cplx *Cg, i
     cp_async_commit();
 }
 
-// ---- C[:, col0 .. col0+32) += Mult (n x 32, sm.panel) * R (32 x 32, sm.R[buf]), in place in L2 -------------
-// warp w owns rows [16 w, 16 w + 16): 2 x 4 DMMA blocks of 8 x 8 complex.
-__device__ __forceinline__ void hs_update_chunk(const HSmem &sm, int buf, cplx *Cg, int ld, int n, int col0, int ncols, int kmax)
+// ---- C[:, col0 .. col0+16) += Mult (n x 32, sm.panel) * R[:, rc0 .. rc0+16) (sm.R[buf]), in place in L2 -----------
+// warp w owns rows [16 w, 16 w + 16); a half-tile is 2 x 2 DMMA blocks of 8 x 8 complex (16 accumulator doubles).
+// Load / compute / store are separate so that the caller can keep the next half-tile's loads in flight while
+// this one is on the tensor pipe (the register budget of 128 has no room for a second full 16 x 32 tile).
+struct HSHalf { double re[2][2][2], im[2][2][2]; };
+
+__device__ __forceinline__ void hs_half_load(HSHalf &h, const cplx *Cg, int ld, int n, int col0, int ncols)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-    const int wr = warp * 16;
-    if (wr >= n) return;
-    double cre[2][4][2], cim[2][4][2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
 #pragma unroll
     for (int i = 0; i < 2; i++) {
-        const int rr = wr + i * 8 + g;
+        const int rr = warp * 16 + i * 8 + g;
         const cplx *src = Cg + (long long)rr * ld + col0 + 2 * t;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-#pragma unroll
-            for (int q = 0; q < 2; q++) {
-                cplx v = cmake(0.0, 0.0);
-                if (rr < n && col0 + j * 8 + 2 * t + q < ncols) v = ldcg(src + j * 8 + q);
-                cre[i][j][q] = v.x; cim[i][j][q] = v.y;
-            }
+        for (int j = 0; j < 2; j++) {
+            // elements (rr, c) and (rr, c + 1), c even: one 32-byte sector, one LDG.256 (two 16-byte loads would each
+            // touch half a sector and double the L2 transactions).  c + 1 may be the padding column (ld is even).
+            double r0 = 0.0, i0 = 0.0, r1 = 0.0, i1 = 0.0;
+            if (rr < n && col0 + j * 8 + 2 * t < ncols) ld256cg(src + j * 8, r0, i0, r1, i1);
+            h.re[i][j][0] = r0; h.im[i][j][0] = i0; h.re[i][j][1] = r1; h.im[i][j][1] = i1;
         }
     }
-    const cplx *cA = sm.panel + wr * HS_LDP;
-    const cplx *cB = sm.R[buf];
+}
+
+__device__ __forceinline__ void hs_half_compute(HSHalf &h, const HSmem &sm, int buf, int rc0)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+    const cplx *cA = sm.panel + warp * 16 * HS_LDP;
+    const cplx *cB = sm.R[buf] + rc0;
+    // always the full K = 32 (Mult columns / R rows beyond the panel width are zero)
 #pragma unroll 2
-    for (int kk = 0; kk < kmax; kk += 4) {
-        cplx a[2], bb[4];
+    for (int kk = 0; kk < HS_B; kk += 4) {
+        cplx a[2], bb[2];
 #pragma unroll
         for (int i = 0; i < 2; i++) a[i] = cA[(i * 8 + g) * HS_LDP + kk + t];
 #pragma unroll
-        for (int j = 0; j < 4; j++) bb[j] = cB[(kk + t) * HS_LDR + j * 8 + g];
+        for (int j = 0; j < 2; j++) bb[j] = cB[(kk + t) * HS_LDR + j * 8 + g];
 #pragma unroll
         for (int i = 0; i < 2; i++) {
             const double nai = -a[i].y;
 #pragma unroll
-            for (int j = 0; j < 4; j++) zmma884(cre[i][j], cim[i][j], a[i].x, a[i].y, nai, bb[j].x, bb[j].y);
+            for (int j = 0; j < 2; j++) zmma884(h.re[i][j], h.im[i][j], a[i].x, a[i].y, nai, bb[j].x, bb[j].y);
         }
     }
+}
+
+__device__ __forceinline__ void hs_half_store(const HSHalf &h, cplx *Cg, int ld, int n, int col0, int ncols)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
 #pragma unroll
     for (int i = 0; i < 2; i++) {
-        const int rr = wr + i * 8 + g;
+        const int rr = warp * 16 + i * 8 + g;
         cplx *dst = Cg + (long long)rr * ld + col0 + 2 * t;
 #pragma unroll
-        for (int j = 0; j < 4; j++)
-#pragma unroll
-            for (int q = 0; q < 2; q++)
-                if (rr < n && col0 + j * 8 + 2 * t + q < ncols) dst[j * 8 + q] = cmake(cre[i][j][q], cim[i][j][q]);
+        for (int j = 0; j < 2; j++)
+            if (rr < n && col0 + j * 8 + 2 * t < ncols) st256(dst + j * 8, h.re[i][j][0], h.im[i][j][0], h.re[i][j][1], h.im[i][j][1]);
     }
 }
 
@@ -290,7 +347,7 @@ __device__ __forceinline__ void hs_update_chunk(const HSmem &sm, int buf, cplx *
 __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof)
 {
     long long tc = prof ? clock64() : 0;
-#define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) prof[slot] += now_ - tc; tc = now_; } } while (0)
+#define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
     const int tid = threadIdx.x;
     bool used = !(tid < n);
     const int nchm = (n + HS_B - 1) / HS_B, ncha = (nc + HS_B - 1) / HS_B;
@@ -305,7 +362,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         cp_async_wait<0>();
         __syncthreads();
         HS_TICK(1);
-        hs_factor_panel(sm, n, k0, bw, used, status_slot);
+        hs_factor_panel(sm, n, k0, bw, used, status_slot, prof);
         HS_TICK(2);
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
         for (int e = tid; e < n * HS_B; e += HS_NT) {
@@ -316,20 +373,35 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
         // chunk list: matrix chunks except the panel's own, then the propagator chunks
         const int skip = k0 / HS_B, total = nchm - 1 + ncha;
-        const int kmax = (bw + 3) & ~3;
         auto chunk = [&](int q, cplx *&base, int &col0, int &ncols) {
             if (q < nchm - 1) { const int j = q < skip ? q : q + 1; base = X; col0 = j * HS_B; ncols = n; }
             else { base = W; col0 = (q - (nchm - 1)) * HS_B; ncols = nc; }
         };
-        cplx *base = nullptr; int col0 = 0, ncols = 0;
-        if (total > 0) { chunk(0, base, col0, ncols); hs_stage_R(sm, 0, base, ld, col0, ncols, bw); }
+        // software pipeline over half-tiles (16 columns): while one half is on the tensor pipe the other half's
+        // C fragments are in flight from L2; R of chunk q+1 is staged while chunk q computes.
+        cplx *base = nullptr, *bnext = nullptr; int col0 = 0, ncols = 0, c2 = 0, n2 = 0;
+        const bool active = (threadIdx.x >> 5) * 16 < n;
+        HSHalf h0, h1;
+        if (total > 0) {
+            chunk(0, base, col0, ncols);
+            hs_stage_R(sm, 0, base, ld, col0, ncols, bw);
+            if (active) hs_half_load(h0, base, ld, n, col0, ncols);
+        }
         HS_TICK(3);
         for (int q = 0; q < total; q++) {
+            if (active) hs_half_load(h1, base, ld, n, col0 + 16, ncols);
             cp_async_wait<0>();
             __syncthreads();
-            if (q + 1 < total) { cplx *b2; int c2, n2; chunk(q + 1, b2, c2, n2); hs_stage_R(sm, (q + 1) & 1, b2, ld, c2, n2, bw); }
-            chunk(q, base, col0, ncols);
-            hs_update_chunk(sm, q & 1, base, ld, n, col0, ncols, kmax);
+            const bool more = q + 1 < total;
+            if (more) { chunk(q + 1, bnext, c2, n2); hs_stage_R(sm, (q + 1) & 1, bnext, ld, c2, n2, bw); }
+            if (active) {
+                hs_half_compute(h0, sm, q & 1, 0);
+                hs_half_store(h0, base, ld, n, col0, ncols);
+                if (more) hs_half_load(h0, bnext, ld, n, c2, n2);
+                hs_half_compute(h1, sm, q & 1, 16);
+                hs_half_store(h1, base, ld, n, col0 + 16, ncols);
+            }
+            base = bnext; col0 = c2; ncols = n2;
         }
         __syncthreads();
         HS_TICK(4);
@@ -469,35 +541,42 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
 {
     extern __shared__ __align__(16) unsigned char hs_smem_raw[];
     HSmem &sm = *reinterpret_cast<HSmem *>(hs_smem_raw);
-    const int bl = blockIdx.x, tid = threadIdx.x, M = a.M, ld = a.ldn, nc = M / 2;
+    const int tid = threadIdx.x, M = a.M, ld = a.ldn, nc = M / 2;
+    const long long unit = (long long)a.unit0 + blockIdx.x;
+    const int bl = (int)(unit % a.nb);
+    const int hs_begin = a.hs_begin + (int)(unit / a.nb) * a.unit_len;
+    const int hs_end = (hs_begin + a.unit_len < a.hs_end) ? hs_begin + a.unit_len : a.hs_end;
+    if (hs_begin >= hs_end) return;
     const long long xs = (long long)ld * ld;
     cplx *Xb[2] = {a.X0 + bl * xs, a.X1 + bl * xs};
     cplx *Wb[2] = {a.P0 + bl * xs, a.P1 + bl * xs};
     int *gperm = a.perm + (long long)bl * HS_NMAX;
     int *status_slot = a.status + bl;
-    if (a.hs_begin > 0) {
+    if (hs_begin > 0) {
         if (tid < HS_NMAX) sm.perm[tid] = gperm[tid];
         __syncthreads();
-        const int hp_ = a.hs_begin - 1, ip = hp_ >> 1, kp = hp_ & 1;
+        const int hp_ = hs_begin - 1, ip = hp_ >> 1, kp = hp_ & 1;
         const int np = half_count(M, kp == 0 ? ((ip + 1) & 1) : (ip & 1));
         if (tid < np) sm.pinv[sm.perm[tid]] = tid;
         __syncthreads();
     }
+    if (tid < 16) sm.prof[tid] = 0;
     int n = 0;
-    for (int hs = a.hs_begin; hs < a.hs_end; hs++) {
+    for (int hs = hs_begin; hs < hs_end; hs++) {
         const int i = hs >> 1, kind = hs & 1, cur = hs & 1;
         if (tid < HS_NMAX) { sm.perm_prev[tid] = sm.perm[tid]; sm.pinv_prev[tid] = sm.pinv[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
         hs_assemble(sm, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
         __syncthreads();
-        if (a.prof && tid == 0) a.prof[bl * 8 + 0] += clock64() - tc0;
+        if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         n = half_count(M, kind == 0 ? ((i + 1) & 1) : (i & 1));
-        hs_gauss_jordan(sm, Xb[cur ^ 1], Wb[cur ^ 1], ld, n, nc, status_slot, a.prof ? a.prof + bl * 8 : nullptr);
+        hs_gauss_jordan(sm, Xb[cur ^ 1], Wb[cur ^ 1], ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr);
     }
     if (tid < HS_NMAX) gperm[tid] = sm.perm[tid];
-    if (a.hs_end > a.hs_begin && (a.g_out || a.P_out)) {
-        const int fin = a.hs_end & 1;                  // buffer written by the last half-step
+    if (a.prof && tid < 16) a.prof[bl * 16 + tid] += sm.prof[tid];
+    if (hs_end == a.hs_end && (a.g_out || a.P_out)) {
+        const int fin = hs_end & 1;                  // buffer written by the last half-step
         const long long os = (long long)a.nh * a.nh;
         if (a.g_out)
             for (int idx = tid; idx < n * n; idx += HS_NT) {

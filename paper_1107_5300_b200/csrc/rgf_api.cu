@@ -477,23 +477,42 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
     static const bool prof_on = getenv("RGF_HS_PROF") != nullptr;          // debugging aid: per-phase cycle counters
     if (prof_on) {
-        if ((rc = ensure(p, p->counters, sizeof(long long) * 8 * (size_t)nb))) return rc;
-        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * 8 * (size_t)nb, w.stream));
+        if ((rc = ensure(p, p->counters, sizeof(long long) * 16 * (size_t)nb))) return rc;
+        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * 16 * (size_t)nb, w.stream));
         a.prof = ptr<long long>(p->counters);
     }
-    half_sweep_kernel<<<nb, HS_NT, sizeof(HSmem), w.stream>>>(a);
+    // Rounds of units: with more matrices than resident CTA slots (2 per SM) a single launch would run 512 matrices
+    // as 296 + 216, the second wave half empty.  Instead every launch runs `slots` units of unit_len half-steps; unit
+    // u = (matrix u % nb, chunk u / nb), so chunk c+1 of a matrix is always in a later launch than its chunk c
+    // (nb > slots) and stream order is the only dependency.
+    int sms = 0, occ = 0;
+    CUDA_TRY(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
+    CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, half_sweep_kernel, HS_NT, sizeof(HSmem)));
+    const int slots = std::max(1, occ) * sms;
+    if (nb <= slots) {
+        a.unit0 = 0; a.unit_len = a.hs_end;
+        half_sweep_kernel<<<nb, HS_NT, sizeof(HSmem), w.stream>>>(a);
+        p->stats.launches++;
+    } else {
+        a.unit_len = std::min(a.hs_end, 64);
+        const long long nchunks = (a.hs_end + a.unit_len - 1) / a.unit_len, units = nchunks * nb;
+        for (long long u0 = 0; u0 < units; u0 += slots) {
+            a.unit0 = (int)u0;
+            half_sweep_kernel<<<(unsigned)std::min<long long>(slots, units - u0), HS_NT, sizeof(HSmem), w.stream>>>(a);
+            p->stats.launches++;
+        }
+    }
+    CUDA_TRY(p, cudaGetLastError());
     if (prof_on) {
-        std::vector<long long> h(8 * (size_t)nb);
+        std::vector<long long> h(16 * (size_t)nb);
         CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->counters.p, sizeof(long long) * h.size(), cudaMemcpyDeviceToHost, w.stream));
         CUDA_TRY(p, cudaStreamSynchronize(w.stream));
-        double s[8] = {0};
-        for (int b = 0; b < nb; b++) for (int k = 0; k < 8; k++) s[k] += (double)h[8 * (size_t)b + k];
+        double s[16] = {0};
+        for (int b = 0; b < nb; b++) for (int k = 0; k < 16; k++) s[k] += (double)h[16 * (size_t)b + k];
         const double hsn = (double)nb * a.hs_end;
-        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f\n",
-                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn);
+        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           update loop: load1 %.0f sync %.0f stageR %.0f comp0 %.0f store0 %.0f load0 %.0f comp1 %.0f store1 %.0f\n",
+                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[8] / hsn, s[9] / hsn, s[10] / hsn, s[11] / hsn, s[12] / hsn, s[13] / hsn, s[14] / hsn, s[15] / hsn);
     }
-    p->stats.launches++;
-    CUDA_TRY(p, cudaGetLastError());
     *g_out = ptr<cplx>(w.H0); *Pcur_out = ptr<cplx>(w.Pa);
     return RGF_OK;
 }
