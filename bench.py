@@ -34,6 +34,10 @@ sys.path.insert(0, ROOT)
 
 from paper_1107_5300_b200 import inputs  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the headline launch configuration,
+# from the ncu --set full capture summarised in profiles/ (bytes; None = not captured for this formulation)
+TRAFFIC_NCU = {"half": 84.75e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
+
 METRIC = "rgf_slice_steps_per_s"
 UNIT = "slice-steps/s"
 
@@ -245,22 +249,32 @@ def main():
     units_step = world * n_E * w.L                        # slice-steps per step over all ranks
     if rank == 0:
         value = units_step * a.steps / (ms_max * 1e-3)
+        fused = a.form == "half" and (w.M + 1) // 2 <= 128          # the fused half_sweep_kernel runs the whole sweep
         n_inv = w.M // 2 if a.form == "half" else w.M          # matrix size of the inverses (M even at the headline)
-        fl_inv, l_inv = update_flops_per_inverse(n_inv)
-        flops_per_launch = fl_inv / max(l_inv, 1) * stats["cohort"]
         avg_ms = ms_upd / max(n_upd, 1)
-        achieved = flops_per_launch / (avg_ms * 1e-3) * 1e-12 if avg_ms > 0 else 0.0
-        if a.form == "half":
-            flops_step = n_E * w.L * 2 * (8.0 * n_inv ** 3 + 8.0 * n_inv ** 3)     # executed: 2 x ((M/2) inverse + (M/2)^3 GEMM)
+        if fused:
+            # algorithmic flops of one half-step: n^3 complex MACs for the in-place Gauss-Jordan inverse + n^2 nc for the
+            # propagator columns that ride along as right-hand sides (8 real flops per complex MAC); 2 half-steps per slice
+            flops_step = n_E * w.L * 2 * (8.0 * n_inv ** 3 + 8.0 * n_inv ** 2 * (w.M // 2))
+            flops_per_launch = flops_step * a.steps / max(n_upd, 1)
+            kernel_name = "half_sweep_kernel (fused assembly + augmented Gauss-Jordan [A | C P], FP64 DMMA.8x8x4)"
         else:
-            flops_step = n_E * w.L * (8.0 * w.M ** 3 + 8.0 * (w.M / 2) ** 3)      # executed: dense inverse + compact propagator
+            fl_inv, l_inv = update_flops_per_inverse(n_inv)
+            flops_per_launch = fl_inv / max(l_inv, 1) * stats["cohort"]
+            kernel_name = "gj32_update_kernel (FP64 DMMA.8x8x4)"
+            if a.form == "half":
+                flops_step = n_E * w.L * 2 * (8.0 * n_inv ** 3 + 8.0 * n_inv ** 3)     # executed: 2 x ((M/2) inverse + (M/2)^3 GEMM)
+            else:
+                flops_step = n_E * w.L * (8.0 * w.M ** 3 + 8.0 * (w.M / 2) ** 3)      # executed: dense inverse + compact propagator
+        achieved = flops_per_launch / (avg_ms * 1e-3) * 1e-12 if avg_ms > 0 else 0.0
+        state_bytes = 4 * (n_inv + (n_inv & 1)) ** 2 * 16 if fused else w.M * w.M * 16
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[2] armchair ribbon M=%d L=%d n_E=%d per GPU, Anderson +-0.1 eV seed 5300, complex128" % (w.M, w.L, n_E),
                        "eta": w.eta, "t": w.t, "cohort": stats["cohort"], "formulation": a.form,
-                       "l2_policy": "inputs larger than L2 (%.0f MB of state per step)" % (stats["cohort"] * w.M * w.M * 16 / 1e6)},
+                       "l2_policy": "inputs larger than L2 (%.0f MB of per-matrix state streamed every slice)" % (stats["cohort"] * state_bytes / 1e6)},
             "energies_per_s": world * n_E * a.steps / (ms_max * 1e-3),
             "tflops_executed": flops_step * world * a.steps / (ms_max * 1e-3) * 1e-12,
             "tflops_dense_equivalent": 16.0 * w.M ** 3 * units_step * a.steps / (ms_max * 1e-3) * 1e-12,
@@ -268,8 +282,8 @@ def main():
             "lead_iterations": stats["lead_iterations"],
             "gpu_launches": launches,
             "clocks": clocks,
-            "roofline": {"bound": "tensor", "kernel": "gj_update_kernel<32> (FP64 DMMA.8x8x4)", "achieved": achieved, "peak": peak,
-                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": None,
+            "roofline": {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": TRAFFIC_NCU.get(a.form) if (w.M, w.L, n_E) == (244, 8000, 512) else None,
                          "peak_source": "measured live: rgf_fp64_peak_tflops (DMMA issue rate, this GPU)",
                          "launches_timed": n_upd, "share_of_step": ms_upd / ms if ms else None},
         }

@@ -91,9 +91,10 @@ typedef struct rgf_stats {
     double ms_leads;            /* lead decimation                                               */
     double ms_sweep;            /* assembly + inverse + propagator over all slices              */
     double ms_trace;            /* Gamma trace + download                                        */
-    double ms_inverse_update;   /* summed CUDA-event time of the Gauss-Jordan update kernel      */
+    double ms_inverse_update;   /* summed CUDA-event time of the dominant kernel of the sweep: the fused
+                                   half_sweep_kernel (RGF_FORM_HALF, M <= 256), else the Gauss-Jordan update   */
     long long launches;         /* kernels launched by the call                                  */
-    long long launches_inverse_update; /* gj_update launches of the sweep (the ones timed)            */
+    long long launches_inverse_update; /* launches of that kernel in the sweep (the ones timed)       */
     long long launches_leads;   /* kernels launched by the lead decimation                       */
     int lead_iterations;        /* decimation iterations run (max over energies)                 */
     int cohort;                 /* matrices per launch                                           */

@@ -489,17 +489,29 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     CUDA_TRY(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
     CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, half_sweep_kernel, HS_NT, sizeof(HSmem)));
     const int slots = std::max(1, occ) * sms;
+    const bool timed = p->profiling > 0 && p->in_sweep;
+    auto launch = [&](unsigned grid) -> int {
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (timed) {
+            int rc2 = update_events(p, w, &e0, &e1);
+            if (rc2) return rc2;
+            CUDA_TRY(p, cudaEventRecord(e0, w.stream));
+        }
+        half_sweep_kernel<<<grid, HS_NT, sizeof(HSmem), w.stream>>>(a);
+        if (timed) CUDA_TRY(p, cudaEventRecord(e1, w.stream));
+        p->stats.launches++;
+        if (p->in_sweep) p->stats.launches_inverse_update++;
+        return RGF_OK;
+    };
     if (nb <= slots) {
         a.unit0 = 0; a.unit_len = a.hs_end;
-        half_sweep_kernel<<<nb, HS_NT, sizeof(HSmem), w.stream>>>(a);
-        p->stats.launches++;
+        if ((rc = launch((unsigned)nb))) return rc;
     } else {
         a.unit_len = std::min(a.hs_end, 64);
         const long long nchunks = (a.hs_end + a.unit_len - 1) / a.unit_len, units = nchunks * nb;
         for (long long u0 = 0; u0 < units; u0 += slots) {
             a.unit0 = (int)u0;
-            half_sweep_kernel<<<(unsigned)std::min<long long>(slots, units - u0), HS_NT, sizeof(HSmem), w.stream>>>(a);
-            p->stats.launches++;
+            if ((rc = launch((unsigned)std::min<long long>(slots, units - u0)))) return rc;
         }
     }
     CUDA_TRY(p, cudaGetLastError());
