@@ -22,6 +22,7 @@
 #include "gj_inverse32.cuh"
 #include "half_kernels.cuh"
 #include "half_sweep.cuh"
+#include "half_sweep_c64.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -44,7 +45,7 @@ struct Ws {
     bool own_stream = false;
     cudaEvent_t done = nullptr;
     Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
-    Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm;                        // half-slice formulation: three compact g buffers, C P, trace scratch
+    Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm, Cp0, Cp1;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
     size_t upd_used = 0;
 };
@@ -66,6 +67,7 @@ struct rgf_plan {
     int nstreams = 1;
     int profiling = 0;
     int formulation = RGF_FORM_HALF;
+    int precision = RGF_C128;                     // of the call in progress
     bool in_sweep = false;                        // update-kernel events are taken for the sweep's inverses only
     rgf_stats stats;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -126,6 +128,7 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
     CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
+    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_c64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HC64Smem)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     p->attrs_set = true;
     return RGF_OK;
@@ -529,8 +532,33 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     return RGF_OK;
 }
 
+// complex64 sweep (half_sweep_c64.cuh): one CTA per matrix for the whole sweep, FP32 FFMA
+int run_sweep_cohort_c64(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
+{
+    int rc;
+    const size_t pb = sizeof(float2) * (size_t)HC_NMAX * HC_NMAX * nb;
+    if ((rc = ensure(p, w.Cp0, pb))) return rc;
+    if ((rc = ensure(p, w.Cp1, pb))) return rc;
+    HC64Args a;
+    memset(&a, 0, sizeof(a));
+    a.M = p->M; a.L = p->L; a.nh = p->nh; a.n_E = n_E; a.bz0 = bz0; a.nb = nb; a.eta = eta; a.t = p->t;
+    a.energies = ptr<double>(p->E); a.onsite = ptr<double>(p->onsite);
+    a.bond = ptr<uint8_t>(p->bond); a.hop = ptr<uint8_t>(p->hop);
+    a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
+    a.P0 = ptr<float2>(w.Cp0); a.P1 = ptr<float2>(w.Cp1);
+    a.status = ptr<int>(p->status) + bz0;
+    a.hs_end = 2 * nslices;
+    a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
+    half_sweep_c64_kernel<<<nb, HC_NT, sizeof(HC64Smem), w.stream>>>(a);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    *g_out = ptr<cplx>(w.H0); *Pcur_out = ptr<cplx>(w.Pa);
+    return RGF_OK;
+}
+
 int run_sweep_cohort_half(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
 {
+    if (p->precision == RGF_C64) return run_sweep_cohort_c64(p, w, n_E, eta, bz0, nb, nslices, g_out, Pcur_out);
     if (use_fused(p)) return run_sweep_cohort_fused(p, w, n_E, eta, bz0, nb, nslices, g_out, Pcur_out);
     const int M = p->M, L = p->L, nh = p->nh, nc = M / 2;
     const long long hs = (long long)nh * nh;
@@ -729,10 +757,10 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     if (rc) return rc;
     if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_transmission before rgf_set_device");
     if (!T_out) return fail(p, RGF_EINVAL, "T_out is NULL");
-    if (precision != RGF_C128) {
-        if (precision == RGF_C64) return fail(p, RGF_EUNSUPPORTED, "complex64 sweep is not built in this version");
-        return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
-    }
+    if (precision != RGF_C128 && precision != RGF_C64) return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
+    if (precision == RGF_C64 && (p->formulation != RGF_FORM_HALF || p->nh > HC_NMAX))
+        return fail(p, RGF_EUNSUPPORTED, "the complex64 sweep is built for RGF_FORM_HALF and M <= 256 only");
+    p->precision = precision;
     memset(&p->stats, 0, sizeof(p->stats));
     for (Ws &w : p->ws) w.upd_used = 0;
     CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
@@ -819,7 +847,7 @@ int rgf_destroy(rgf_plan *p)
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
-        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm};
+        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm, &w.Cp0, &w.Cp1};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
         if (w.done) cudaEventDestroy(w.done);
@@ -972,7 +1000,10 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     if (rc) return rc;
     if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_sweep_state before rgf_set_device");
     if (dev < 0 || dev >= p->n_dev || nslices < 1 || nslices > p->L || !g_out || !P_out) return fail(p, RGF_EINVAL, "bad argument");
-    if (precision != RGF_C128) return fail(p, RGF_EUNSUPPORTED, "only RGF_C128 is built in this version");
+    if (precision != RGF_C128 && precision != RGF_C64) return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
+    if (precision == RGF_C64 && (p->formulation != RGF_FORM_HALF || p->nh > HC_NMAX))
+        return fail(p, RGF_EUNSUPPORTED, "the complex64 sweep is built for RGF_FORM_HALF and M <= 256 only");
+    p->precision = precision;
     memset(&p->stats, 0, sizeof(p->stats));
     if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
     const int batch = p->n_dev * n_E, M = p->M, nh = p->nh;

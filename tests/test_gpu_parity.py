@@ -205,3 +205,47 @@ def test_errors(rgf, plan):
     with pytest.raises(rgf.RgfError) as e:
         rgf.rgf_set_device(plan.handle, 1, 4, np.zeros((4, 1)), -2.7)
     assert e.value.code == rgf.RGF_EINVAL
+
+
+# ---- complex64 sweep (configs[3] precision study; reading R13) ---------------------------
+
+@pytest.mark.parametrize("M,L,W", [(20, 40, 0.0), (21, 17, 0.3), (64, 50, 0.1), (244, 30, 0.1)])
+def test_c64_sweep_close_to_c128_and_oracle(rgf, plan, oracle, M, L, W):
+    """north_star: the complex64 path stays within |dT| <= 1e-3 outside |E| < 0.1 eV."""
+    on = inputs.anderson(M, L, W, 77 + M) if W > 0 else np.zeros((L, M))
+    E = np.concatenate([np.linspace(-1.0, -0.1, 6), np.linspace(0.1, 1.0, 6)]) + 0.0037
+    plan.set_device(on, -2.7)
+    T128 = plan.transmission(E, 1e-9)[0]
+    T64 = plan.transmission(E, 1e-9, precision=rgf.RGF_C64)[0]
+    assert np.all(np.isfinite(T64))
+    assert np.max(np.abs(T64 - T128)) <= 1e-3, np.abs(T64 - T128)
+    assert np.max(np.abs(T64 - T128)) > 0.0            # it really ran in another precision
+    if M <= 64:
+        T_or = oracle.transmission_batch(on, None, -2.7, E, 1e-9)
+        assert np.max(np.abs(T64 - T_or)) <= 1e-3
+
+
+def test_c64_sweep_state_matches_oracle_to_single_precision(rgf, plan, oracle):
+    M, L, ns = 50, 9, 6
+    on = inputs.anderson(M, L, 0.25, 5)
+    plan.set_device(on, -2.7)
+    E = np.array([-0.8, 0.31])
+    g = np.empty((2, M, M), dtype=complex)
+    P = np.empty((2, M, M), dtype=complex)
+    rgf.rgf_sweep_state(plan.handle, 0, E, 2, 1e-9, rgf.RGF_C64, ns, g, P)
+    for k, e in enumerate(E):
+        g0, P0 = oracle.sweep_state(on, None, -2.7, e, 1e-9, ns)
+        hg = ~np.isnan(g[k].real)
+        assert hg.sum() == (M // 2) ** 2
+        assert np.max(np.abs(g[k][hg] - g0[hg])) < 2e-4 * np.max(np.abs(g0))
+        hp = ~np.isnan(P[k].real)
+        assert np.max(np.abs(P[k][hp] - P0[hp])) < 2e-4 * np.max(np.abs(P0))
+        assert np.max(np.abs(g[k][hg] - g0[hg])) > 1e-12 * np.max(np.abs(g0))      # single precision, not double
+
+
+def test_c64_needs_half_formulation(rgf, plan):
+    plan.set_device(np.zeros((4, 6)), -2.7)
+    rgf.rgf_set_formulation(plan.handle, rgf.RGF_FORM_DENSE)
+    with pytest.raises(rgf.RgfError) as e:
+        plan.transmission(np.array([0.3]), 1e-9, precision=rgf.RGF_C64)
+    assert e.value.code == rgf.RGF_EUNSUPPORTED
