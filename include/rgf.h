@@ -121,8 +121,9 @@ int rgf_set_profiling(rgf_plan *p, int level);
 enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1, RGF_FORM_HALF_STEPWISE = 2 };
 int rgf_set_formulation(rgf_plan *p, int formulation);
 
-/* Matrices per kernel launch in the sweep (0 = library default = the whole batch).  The sweep runs
- * cohort after cohort over all slices; a cohort whose state fits the 126 MB L2 keeps it there. */
+/* Matrices per kernel launch in the sweep (0 = library default).  RGF_FORM_DENSE / _STEPWISE: the sweep runs cohort
+ * after cohort over all slices.  RGF_FORM_HALF (fused kernel): upper bound on the units (matrix, 64 half-steps) per
+ * launch, default = the number of resident CTA slots of the GPU. */
 int rgf_set_cohort(rgf_plan *p, int cohort);
 
 /* Measures the FP64 tensor-pipe ceiling of the plan's GPU (independent DMMA.8x8x4 chains on every

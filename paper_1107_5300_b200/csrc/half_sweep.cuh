@@ -98,8 +98,29 @@ __device__ __forceinline__ double hs_rcp(double v)
 __device__ long long hs_dbg[8];
 #endif
 
-// barrier among the first nthreads threads of the CTA (whole warps); id 1 (0 is __syncthreads)
-__device__ __forceinline__ void hs_bar_active(int nthreads) { asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory"); }
+// named barrier over `nthreads` threads (whole warps)
+__device__ __forceinline__ void hs_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// The panel factorisation is written against a view of the shared-memory buffers and a description of the thread
+// group that runs it (the whole CTA in the kernel below; a warp-specialised variant with four factor warps on one SM
+// sub-partition and twelve update warps was measured 1.35x slower in round 1 and is not shipped: DESIGN.md section 9).
+struct HSView {
+    cplx *panel;          // [HS_NMAX][HS_LDP]
+    cplx *Rs;             // [HS_SB][HS_LDR] snapshot of a sub-block's pivot rows
+    cplx *crow, *cinv;    // candidate buffers [2][8][HS_SB], [2][8]
+    unsigned *ckey;       // [2][8], 16-byte aligned
+    int *prow, *perm, *pinv;
+    long long *prof;      // shared-memory cycle counters or NULL
+};
+struct HSGroup {
+    int r;                // row owned by this thread
+    int slot, nslots;     // candidate slot of this warp, number of warps that search
+    int gtid, gnt;        // thread index inside the group, group size
+    int bar_pivot, n_pivot;   // barrier of the searching warps
+    int bar_all;          // barrier of the whole group (gnt threads)
+    int rbase;            // first of the 32 rows this warp updates in the in-panel DMMAs
+    int nbsel, nbmod;     // ... for the column blocks whose running index % nbmod == nbsel
+};
 
 // One pivot step on column CC (static) of the thread's 8-column sub-block.  Candidate buffers alternate with
 // the parity of CC, so one barrier per column suffices.  32-bit key = top 24 bits of |x|^2 (sign, exponent,
@@ -107,9 +128,9 @@ __device__ __forceinline__ void hs_bar_active(int nthreads) { asm volatile("bar.
 // so the key is unique, names the row, and the lowest row wins ties.  The pivot row is not a divergent branch:
 //   row[j] <- c + a * pivrow[j]   with (a, c) = (d, 0) on the pivot row and (-x d, row[j]) elsewhere, row[CC] <- a.
 template <int CC>
-__device__ __forceinline__ void hs_pivot_step(HSmem &sm, cplx (&row)[HS_SB], bool &used, int r, int warp, int naw,
-                                              int kglob, int *status_slot)
+__device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &gr, cplx (&row)[HS_SB], bool &used, int kglob, int *status_slot)
 {
+    const int r = gr.r, warp = gr.slot, naw = gr.nslots;
     constexpr int SB = HS_SB, NW = HS_NT / 32;
     constexpr int pb = (CC & 1) * NW;
 #ifdef HS_DBG
@@ -135,7 +156,7 @@ __device__ __forceinline__ void hs_pivot_step(HSmem &sm, cplx (&row)[HS_SB], boo
         for (int j = 0; j < SB; j++) if (j != CC) sm.crow[(pb + warp) * SB + j] = row[j];
     }
     HS_DBGT(1);
-    hs_bar_active(naw * 32);
+    hs_bar(gr.bar_pivot, gr.n_pivot);
     HS_DBGT(2);
     const uint4 k4 = *reinterpret_cast<const uint4 *>(&sm.ckey[pb]);
     unsigned best = k4.x;
@@ -179,21 +200,20 @@ __device__ __forceinline__ void hs_pivot_step(HSmem &sm, cplx (&row)[HS_SB], boo
 // ---- panel factorisation in shared memory: columns [k0, k0 + bw) of all n rows --------------------
 // On entry sm.panel[r][c] = X[r][k0 + c] (zero for c >= bw, r >= n).  On exit sm.panel = N' (the
 // transformed columns), sm.prow[c] = pivot row of column k0 + c, perm / pinv updated, used |= pivot.
-__device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw, bool &used, int *status_slot, long long *prof)
+__device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup &gr, int n, int k0, int bw, bool &used, int *status_slot)
 {
-    long long tp = prof ? clock64() : 0;
-    constexpr int B = HS_B, SB = HS_SB, NT = HS_NT, LDP = HS_LDP, LDR = HS_LDR;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-    const int r = tid;
+    constexpr int B = HS_B, SB = HS_SB, LDP = HS_LDP, LDR = HS_LDR;
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const int r = gr.r;
     const bool has_row = r < n;
-    const int naw = (n + 31) >> 5;              // warps that own rows: only they take part in the pivot search
+    long long tp = sm.prof ? clock64() : 0;
     cplx *panel = sm.panel;
-    cplx *Rs = sm.R[0];                       // [SB][LDR] snapshot of the sub-block's pivot rows
+    cplx *Rs = sm.Rs;
     for (int s = 0; s < B / SB; s++) {
         const int c0 = s * SB;
         const int ncols = bw - c0 < SB ? bw - c0 : SB;
         if (ncols <= 0) break;
-        if (prof) tp = clock64();
+        if (sm.prof) tp = clock64();
         cplx row[SB];
         if (has_row) {
 #pragma unroll
@@ -202,33 +222,33 @@ __device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw
 #pragma unroll
             for (int j = 0; j < SB; j++) row[j] = cmake(0.0, 0.0);
         }
-        if (warp < naw) {
+        if (gr.slot < gr.nslots) {
             const int kg = k0 + c0;
-            hs_pivot_step<0>(sm, row, used, r, warp, naw, kg, status_slot);
-            if (ncols > 1) hs_pivot_step<1>(sm, row, used, r, warp, naw, kg + 1, status_slot);
-            if (ncols > 2) hs_pivot_step<2>(sm, row, used, r, warp, naw, kg + 2, status_slot);
-            if (ncols > 3) hs_pivot_step<3>(sm, row, used, r, warp, naw, kg + 3, status_slot);
-            if (ncols > 4) hs_pivot_step<4>(sm, row, used, r, warp, naw, kg + 4, status_slot);
-            if (ncols > 5) hs_pivot_step<5>(sm, row, used, r, warp, naw, kg + 5, status_slot);
-            if (ncols > 6) hs_pivot_step<6>(sm, row, used, r, warp, naw, kg + 6, status_slot);
-            if (ncols > 7) hs_pivot_step<7>(sm, row, used, r, warp, naw, kg + 7, status_slot);
+            hs_pivot_step<0>(sm, gr, row, used, kg, status_slot);
+            if (ncols > 1) hs_pivot_step<1>(sm, gr, row, used, kg + 1, status_slot);
+            if (ncols > 2) hs_pivot_step<2>(sm, gr, row, used, kg + 2, status_slot);
+            if (ncols > 3) hs_pivot_step<3>(sm, gr, row, used, kg + 3, status_slot);
+            if (ncols > 4) hs_pivot_step<4>(sm, gr, row, used, kg + 4, status_slot);
+            if (ncols > 5) hs_pivot_step<5>(sm, gr, row, used, kg + 5, status_slot);
+            if (ncols > 6) hs_pivot_step<6>(sm, gr, row, used, kg + 6, status_slot);
+            if (ncols > 7) hs_pivot_step<7>(sm, gr, row, used, kg + 7, status_slot);
         }
-        __syncthreads();
-        if (prof) { long long now_ = clock64(); if (tid == 0) sm.prof[5] += now_ - tp; tp = now_; }
+        hs_bar(gr.bar_all, gr.gnt);
+        if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[5] += now_ - tp; tp = now_; }
         if (has_row) {
 #pragma unroll
             for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
         }
         const int nbmax = (bw + 7) / 8;
         if (nbmax > 1) {
-            for (int e = tid; e < SB * B; e += NT) {
+            for (int e = gr.gtid; e < SB * B; e += gr.gnt) {
                 const int k = e / B, c = e % B;
                 if (c < c0 || c >= c0 + SB) Rs[k * LDR + c] = (k < ncols) ? panel[sm.prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
             }
-            __syncthreads();
-            // other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs (8 x |J|) on DMMA.
-            // warp -> 32 rows (warp & 3), column blocks of parity (warp >> 2)
-            const int rbase = (warp & 3) * 32;
+            hs_bar(gr.bar_all, gr.gnt);
+            // other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs (8 x |J|) on DMMA; a warp takes 32 rows
+            // and the column blocks whose running index % nbmod == nbsel
+            const int rbase = gr.rbase;
             if (rbase < n) {
                 int pk[2];
 #pragma unroll
@@ -245,7 +265,7 @@ __device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw
                 int cnt = 0;
                 for (int nb = 0; nb < nbmax; nb++) {
                     if (nb == s) continue;
-                    if (((cnt++) & 1) != (warp >> 2)) continue;
+                    if (((cnt++) % gr.nbmod) != gr.nbsel) continue;
                     double cre[4][2], cim[4][2];
                     cplx *Cw = panel + rbase * LDP + nb * 8;
 #pragma unroll
@@ -266,9 +286,27 @@ __device__ __forceinline__ void hs_factor_panel(HSmem &sm, int n, int k0, int bw
                     }
                 }
             }
-            __syncthreads();
+            hs_bar(gr.bar_all, gr.gnt);
         }
     }
+}
+
+// view / group of the whole-CTA kernel: thread = row, all eight warps in the in-panel DMMAs
+__device__ __forceinline__ HSView hs_view(HSmem &sm, bool prof)
+{
+    HSView v;
+    v.panel = sm.panel; v.Rs = sm.R[0]; v.crow = sm.crow; v.cinv = sm.cinv; v.ckey = sm.ckey;
+    v.prow = sm.prow; v.perm = sm.perm; v.pinv = sm.pinv; v.prof = prof ? sm.prof : nullptr;
+    return v;
+}
+__device__ __forceinline__ HSGroup hs_group_cta(int n)
+{
+    HSGroup g;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    g.r = tid; g.slot = warp; g.nslots = (n + 31) >> 5; g.gtid = tid; g.gnt = HS_NT;
+    g.bar_pivot = 1; g.n_pivot = g.nslots * 32; g.bar_all = 0;
+    g.rbase = (warp & 3) * 32; g.nbsel = warp >> 2; g.nbmod = 2;
+    return g;
 }
 
 // ---- R = C[prow[0..bw)][col0 .. col0+32) -> shared memory (cp.async.cg: L2, never a stale L1 line) --------
@@ -308,14 +346,14 @@ __device__ __forceinline__ void hs_half_load(HSHalf &h, const cplx *Cg, int ld, 
     }
 }
 
-__device__ __forceinline__ void hs_half_compute(HSHalf &h, const HSmem &sm, int buf, int rc0)
+__device__ __forceinline__ void hs_half_compute(HSHalf &h, const HSmem &sm, int buf, int rc0, int kmax)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
     const cplx *cA = sm.panel + warp * 16 * HS_LDP;
     const cplx *cB = sm.R[buf] + rc0;
-    // always the full K = 32 (Mult columns / R rows beyond the panel width are zero)
+    // kmax = panel width rounded up to 4 (Mult columns / R rows beyond the panel width are zero)
 #pragma unroll 2
-    for (int kk = 0; kk < HS_B; kk += 4) {
+    for (int kk = 0; kk < kmax; kk += 4) {
         cplx a[2], bb[2];
 #pragma unroll
         for (int i = 0; i < 2; i++) a[i] = cA[(i * 8 + g) * HS_LDP + kk + t];
@@ -350,6 +388,8 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
 #define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
     const int tid = threadIdx.x;
     bool used = !(tid < n);
+    const HSView view = hs_view(sm, prof != nullptr);
+    const HSGroup grp = hs_group_cta(n);
     const int nchm = (n + HS_B - 1) / HS_B, ncha = (nc + HS_B - 1) / HS_B;
     for (int k0 = 0; k0 < n; k0 += HS_B) {
         const int bw = (n - k0 < HS_B) ? (n - k0) : HS_B;
@@ -362,7 +402,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         cp_async_wait<0>();
         __syncthreads();
         HS_TICK(1);
-        hs_factor_panel(sm, n, k0, bw, used, status_slot, prof);
+        hs_factor_panel(view, grp, n, k0, bw, used, status_slot);
         HS_TICK(2);
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
         for (int e = tid; e < n * HS_B; e += HS_NT) {
@@ -373,6 +413,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
         // chunk list: matrix chunks except the panel's own, then the propagator chunks
         const int skip = k0 / HS_B, total = nchm - 1 + ncha;
+        const int kmax = (bw + 3) & ~3;
         auto chunk = [&](int q, cplx *&base, int &col0, int &ncols) {
             if (q < nchm - 1) { const int j = q < skip ? q : q + 1; base = X; col0 = j * HS_B; ncols = n; }
             else { base = W; col0 = (q - (nchm - 1)) * HS_B; ncols = nc; }
@@ -395,10 +436,10 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
             const bool more = q + 1 < total;
             if (more) { chunk(q + 1, bnext, c2, n2); hs_stage_R(sm, (q + 1) & 1, bnext, ld, c2, n2, bw); }
             if (active) {
-                hs_half_compute(h0, sm, q & 1, 0);
+                hs_half_compute(h0, sm, q & 1, 0, kmax);
                 hs_half_store(h0, base, ld, n, col0, ncols);
                 if (more) hs_half_load(h0, bnext, ld, n, c2, n2);
-                hs_half_compute(h1, sm, q & 1, 16);
+                hs_half_compute(h1, sm, q & 1, 16, kmax);
                 hs_half_store(h1, base, ld, n, col0 + 16, ncols);
             }
             base = bnext; col0 = c2; ncols = n2;
@@ -412,9 +453,11 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
 // ---- assembly of A (into Xn) and of W = C P_prev (into Wn) for half-step (i, kind) -------------------------
 // g_prev[k][m] = Xp[perm_prev[k]][pinv_prev[m]], P_prev[k][:] = Wp[perm_prev[k]][:]; blocks of 32 output rows,
 // the physical rows they need staged in the (idle) panel buffer so that every L2 read is a full row.
-__device__ __forceinline__ void hs_assemble(HSmem &sm, const HSweepArgs &a, int bl, int i, int kind, bool first,
+template <class SM, int NT>
+__device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl, int i, int kind, bool first,
                                             const cplx *Xp, const cplx *Wp, cplx *Xn, cplx *Wn)
 {
+    constexpr int HS_NT = NT;        // threads that run the assembly (the whole CTA of either kernel)
     const int tid = threadIdx.x, M = a.M, L = a.L, ld = a.ldn, nc = M / 2;
     const int bz = a.bz0 + bl, d = bz / a.n_E, e = bz % a.n_E;
     const double t2 = a.t * a.t, E = a.energies[e];
@@ -567,7 +610,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         if (tid < HS_NMAX) { sm.perm_prev[tid] = sm.perm[tid]; sm.pinv_prev[tid] = sm.pinv[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
-        hs_assemble(sm, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
+        hs_assemble<HSmem, 256>(sm, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
         __syncthreads();
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         n = half_count(M, kind == 0 ? ((i + 1) & 1) : (i & 1));

@@ -491,7 +491,8 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     int sms = 0, occ = 0;
     CUDA_TRY(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
     CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, half_sweep_kernel, HS_NT, sizeof(HSmem)));
-    const int slots = std::max(1, occ) * sms;
+    int slots = std::max(1, occ) * sms;
+    if (p->cohort_override > 0) slots = std::min(slots, p->cohort_override);      // rgf_set_cohort: fewer units per launch
     const bool timed = p->profiling > 0 && p->in_sweep;
     auto launch = [&](unsigned grid) -> int {
         cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -249,3 +249,32 @@ def test_c64_needs_half_formulation(rgf, plan):
     with pytest.raises(rgf.RgfError) as e:
         plan.transmission(np.array([0.3]), 1e-9, precision=rgf.RGF_C64)
     assert e.value.code == rgf.RGF_EUNSUPPORTED
+
+
+def test_fused_kernel_unit_rounds(rgf, plan, oracle):
+    """The fused kernel runs in rounds of units (matrix, 64 half-steps) when there are more matrices than CTA slots: force
+    3 slots for 2 devices x 5 energies and 3 chunks of half-steps, so that every matrix is resumed twice from the state
+    (X, W, perm) it left in HBM, by a different CTA each time."""
+    M, L = 21, 70
+    on = np.stack([inputs.anderson(M, L, 0.3, 41), inputs.anderson(M, L, 0.3, 42)])
+    E = np.array([-1.3, -0.41, 0.07, 0.66, 1.9])
+    plan.set_device(on, -2.7)
+    T_ref = np.stack([oracle.transmission_batch(on[d], None, -2.7, E, 1e-9) for d in range(2)])
+    for slots in (3, 4, 0):
+        rgf.rgf_set_cohort(plan.handle, slots)
+        T = plan.transmission(E, 1e-9)
+        assert np.all(np.abs(T - T_ref) <= tol(T_ref)), (slots, np.max(np.abs(T - T_ref)))
+    rgf.rgf_set_cohort(plan.handle, 3)
+    assert plan.stats()["launches"] > 0
+
+
+@pytest.mark.parametrize("M,L", [(21, 9), (32, 12)])
+def test_c64_with_vacancies_and_odd_width(rgf, plan, oracle, M, L):
+    on = inputs.anderson(M, L, 0.2, 7 * M)
+    vac = inputs.edge_vacancies(M, L, 0.3, 11)
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.array([-1.4, -0.6, 0.35, 1.1])
+    plan.set_device(on, -2.7, vac)
+    T64 = plan.transmission(E, 1e-9, precision=rgf.RGF_C64)[0]
+    T_or = oracle.transmission_batch(on, vac, -2.7, E, 1e-9)
+    assert np.max(np.abs(T64 - T_or)) <= 1e-3, np.abs(T64 - T_or)
