@@ -121,6 +121,17 @@ int rgf_set_profiling(rgf_plan *p, int level);
 enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1, RGF_FORM_HALF_STEPWISE = 2 };
 int rgf_set_formulation(rgf_plan *p, int formulation);
 
+/* How the Sancho-Rubio decimation of the clean two-slice lead cell (BASELINE.json:north_star item 4) inverts the cell:
+ *   RGF_LEAD_CELL_DENSE  one pivoted 2M x 2M inverse per iteration + 8 products of size M;
+ *   RGF_LEAD_CELL_SCHUR  (default) the same iteration on the (M/2)-blocks alpha, beta and the corrections really
+ *                        occupy; the four corner blocks of the cell's inverse it consumes come from one pivoted inverse
+ *                        of the M x M Schur complement on the atoms that bond to the neighbouring cells (the other
+ *                        atoms pair up across the two slices and are eliminated in closed form): 8x fewer flops.
+ *                        Falls back to RGF_LEAD_CELL_DENSE for a call with an energy within 1 % of +-t, where the
+ *                        closed elimination is resonant.  Both give the same surface Green's function (tested). */
+enum { RGF_LEAD_CELL_DENSE = 0, RGF_LEAD_CELL_SCHUR = 1 };
+int rgf_set_lead_method(rgf_plan *p, int method);
+
 /* Matrices per kernel launch in the sweep (0 = library default).  RGF_FORM_DENSE / _STEPWISE: the sweep runs cohort
  * after cohort over all slices.  RGF_FORM_HALF (fused kernel): upper bound on the units (matrix, 64 half-steps) per
  * launch, default = the number of resident CTA slots of the GPU. */

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "librgf_b200.so")
 
 RGF_C128, RGF_C64 = 0, 1
 RGF_FORM_DENSE, RGF_FORM_HALF, RGF_FORM_HALF_STEPWISE = 0, 1, 2
+RGF_LEAD_CELL_DENSE, RGF_LEAD_CELL_SCHUR = 0, 1
 RGF_OK, RGF_EINVAL, RGF_ECUDA, RGF_ENOMEM, RGF_ENOCONV, RGF_ESINGULAR, RGF_ESTATE, RGF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7
 
 if not os.path.exists(LIB_PATH):
@@ -41,6 +42,7 @@ _lib.rgf_get_stats.argtypes = [_vp, C.POINTER(rgf_stats)]
 _lib.rgf_set_profiling.argtypes = [_vp, C.c_int]
 _lib.rgf_set_cohort.argtypes = [_vp, C.c_int]
 _lib.rgf_set_formulation.argtypes = [_vp, C.c_int]
+_lib.rgf_set_lead_method.argtypes = [_vp, C.c_int]
 _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
@@ -114,6 +116,10 @@ def rgf_set_profiling(plan, level):
 
 def rgf_set_formulation(plan, formulation):
     return _check(plan, _lib.rgf_set_formulation(plan, formulation))
+
+
+def rgf_set_lead_method(plan, method):
+    return _check(plan, _lib.rgf_set_lead_method(plan, method))
 
 
 def rgf_set_cohort(plan, cohort):

@@ -506,20 +506,38 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
         }
     }
     __syncthreads();
-    for (int r0 = 0; r0 < n; r0 += 32) {
-        const int r1 = (r0 + 32 < n) ? r0 + 32 : n;
-        int slo = r0, shi = r1 - 1;
+    // blocks of 16 output rows; the (<= 18) physical rows a block needs are staged by cp.async into one of two areas of
+    // the panel buffer, the next block's rows in flight while this block is computed
+    constexpr int RB = 16, AREA = (RB + 2) * HS_NMAX;
+    static_assert(2 * AREA <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
+    auto rows_of = [&](int r0, int &slo, int &nst) {
+        const int r1 = (r0 + RB < n) ? r0 + RB : n;
+        int shi = r1 - 1;
+        slo = r0;
         if (kind == 1) { if (par == 0) slo = r0 - 1; else shi = r1; }
         if (slo < 0) slo = 0;
         if (shi > nprev - 1) shi = nprev - 1;
-        const int nst = shi - slo + 1;
+        nst = shi - slo + 1;
+    };
+    auto stage_rows = [&](int r0, int area) {
+        int slo, nst;
+        rows_of(r0, slo, nst);
+        cplx *dst = stage + area * AREA;
         for (int idx = tid; idx < nst * ld; idx += HS_NT) {
             const int sl = idx / ld, c = idx - sl * ld;
-            cp_async16(stage + sl * HS_NMAX + c, Xp + (long long)sm.perm_prev[slo + sl] * ld + c, 16);
+            cp_async16(dst + sl * HS_NMAX + c, Xp + (long long)sm.perm_prev[slo + sl] * ld + c, 16);
         }
         cp_async_commit();
-        cp_async_wait<0>();
+    };
+    stage_rows(0, 0);
+    for (int r0 = 0, blk = 0; r0 < n; r0 += RB, blk++) {
+        const int r1 = (r0 + RB < n) ? r0 + RB : n;
+        int slo, nst;
+        rows_of(r0, slo, nst);
+        if (r0 + RB < n) { stage_rows(r0 + RB, (blk + 1) & 1); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
         __syncthreads();
+        const cplx *st = stage + (blk & 1) * AREA;
         for (int idx = tid; idx < (r1 - r0) * n; idx += HS_NT) {
             const int rl = idx / n, c = idx - rl * n, r = r0 + rl;
             cplx v = cmake(0.0, 0.0);
@@ -527,16 +545,16 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
             const int ca = tb.ca[c], cb = tb.cb[c];
             double sx = 0.0, sy = 0.0;
             if (kind == 0) {
-                if (tb.ra[r] && ca >= 0) { const cplx g = stage[(r - slo) * HS_NMAX + ca]; sx = g.x; sy = g.y; }
+                if (tb.ra[r] && ca >= 0) { const cplx g = st[(r - slo) * HS_NMAX + ca]; sx = g.x; sy = g.y; }
             } else {
                 const int ua = tb.ra[r], ub = tb.rb[r];
                 if (ua >= 0) {
-                    const cplx *sr = stage + (ua - slo) * HS_NMAX;
+                    const cplx *sr = st + (ua - slo) * HS_NMAX;
                     if (ca >= 0) { const cplx g = sr[ca]; sx += g.x; sy += g.y; }
                     if (cb >= 0) { const cplx g = sr[cb]; sx += g.x; sy += g.y; }
                 }
                 if (ub >= 0) {
-                    const cplx *sr = stage + (ub - slo) * HS_NMAX;
+                    const cplx *sr = st + (ub - slo) * HS_NMAX;
                     if (ca >= 0) { const cplx g = sr[ca]; sx += g.x; sy += g.y; }
                     if (cb >= 0) { const cplx g = sr[cb]; sx += g.x; sy += g.y; }
                 }
@@ -550,13 +568,14 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
         }
         __syncthreads();
     }
-    // W = C P_prev: coalesced rows straight from L2, 4 independent elements per thread in flight
+    // W = C P_prev: coalesced rows straight from L2, 6 independent elements per thread in flight
     const int nel = n * nc;
-    for (int base = 0; base < nel; base += 4 * HS_NT) {
-        cplx va[4], vb[4];
-        int rr[4], cc[4];
+    constexpr int WB = 6;
+    for (int base = 0; base < nel; base += WB * HS_NT) {
+        cplx va[WB], vb[WB];
+        int rr[WB], cc[WB];
 #pragma unroll
-        for (int k = 0; k < 4; k++) {
+        for (int k = 0; k < WB; k++) {
             const int idx = base + k * HS_NT + tid;
             va[k] = cmake(0.0, 0.0); vb[k] = cmake(0.0, 0.0);
             rr[k] = -1;
@@ -573,7 +592,7 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
             }
         }
 #pragma unroll
-        for (int k = 0; k < 4; k++)
+        for (int k = 0; k < WB; k++)
             if (rr[k] >= 0) Wn[(long long)rr[k] * ld + cc[k]] = cmake(a.t * (va[k].x + vb[k].x), a.t * (va[k].y + vb[k].y));
     }
     __syncthreads();          // the tables alias the pivot-search buffers

@@ -61,8 +61,10 @@ struct rgf_plan {
     Buf E, T, status, lead_flags, counters;       // per call
     std::vector<Ws> ws;                           // ws[0] runs on the plan's stream
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
-    Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_T4, l_W, l_W2;   // decimation workspace
+    Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
+    Buf lc_S3, lc_R;                              // run_lead_side_schur: S again and the residual of its inverse
+    int fast_leads = 1;
     int cohort_override = 0;
     int nstreams = 1;
     int profiling = 0;
@@ -277,89 +279,156 @@ int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *
 
 namespace {
 
-// ------------------------------------------------------------------------------------------
-// A2. Lead surface Green's functions g_L (slice -1) and g_R (slice L) for n_E energies.
-// Sancho-Rubio decimation on the clean two-slice lead cell (BASELINE.json:north_star item 4):
-//   g = (z - eps)^-1; eps_s += (towards the bulk); eps += a g b + b g a; a <- a g a; b <- b g b
-// on the 2M x 2M cell until max|a|, max|b| < 1e-14 eV for every energy (cap 64 iterations).
+// A2. Lead surface Green's functions g_L (slice -1) and g_R (slice L) for n_E energies (BASELINE.json:north_star item 4).
 // side -1: V_a = t diag(m_{-2}), V_b = t diag(m_{-1});  side +1: V_a = t diag(m_L), V_b = t diag(m_{L+1}).
+
+// ------------------------------------------------------------------------------------------
+// A2.  Sancho-Rubio decimation of the clean two-slice lead cell (pa, pb = slice indices of the cell, V_a = t diag(m_pa)
+// inside the cell, V_b = t diag(m_pb) to the next cell) for n_E energies; writes the surface Green's function on the
+// atoms that bond to the device into g_out [n_E][M][M] (zero elsewhere).
+//   g = (z - eps)^-1; eps_s += (towards the bulk); eps += a g b + b g a; a <- a g a; b <- b g b   until max|a| < 1e-14 eV
+// (1) alpha = h01 lives on the block (o, e), beta = alpha^T on (e, o) and the corrections of eps on X = (o, o) and
+//     Y = (e, e), where e / o are the nc = M/2 atoms of the cell's first / second slice that bond to the neighbouring
+//     cells (parity of pb) -- alpha g alpha etc. never leave these blocks -- so the iteration is carried on nc x nc
+//     matrices and consumes only the corner blocks g[e,e], g[e,o], g[o,o] of the cell's inverse.
+// (2) beta = alpha^T is kept structurally (only alpha is iterated) and g, X, Y are symmetrised: the decimation
+//     squares alpha while |alpha| is O(1..100) for ~30 iterations and amplifies an antisymmetric rounding component
+//     until it diverges at some energies (E = 0.4637 eV at M = 244 with alpha and beta iterated separately).
+// (3) The corner blocks come either from the pivoted inverse of the whole 2M x 2M cell (dense = true) or from the
+//     pivoted inverse of the 2nc x 2nc Schur complement on (e, o): the other atoms f (first slice) and b (second) bond
+//     pairwise, f_j -- b_j with t, and to nothing else among themselves, so their block is [[z, -t], [-t, z]] (x) I
+//     with the closed inverse [[z, t], [t, z]] / (z^2 - t^2) and
+//         S = [[z - Y - k1 K, -k2 K], [-k2 K, z - X - k1 K]],  k1 = z / (z^2 - t^2),  k2 = t / (z^2 - t^2),
+//     K[r][c] = t^2 * #(atoms adjacent to both corner atoms r and c): 8x fewer flops; resonant only at E = +-t, where
+//     the caller takes the dense route.  The inverse of S gets one Newton step (the decimation amplifies its residual).
 // ------------------------------------------------------------------------------------------
 constexpr double kLeadTol = 1e-14;
 constexpr int kLeadMaxIt = 64;
 
-// C (M x M, ld = M) = A (M x M, ld lda) * B (M x M, ld ldb), batched over n_E
-int lead_gemm(rgf_plan *p, const cplx *A, int lda, long long a_batch, const cplx *B, int ldb, long long b_batch, cplx *C, int n_E)
+int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, bool dense, cplx *g_out, int *iters_out, int *n_open_out)
 {
-    const int M = p->M;
-    ZgemmArgs a;
-    memset(&a, 0, sizeof(a));
-    a.A = A; a.a_batch = a_batch; a.a_rs = lda; a.a_cs = 1; a.kmask_div = 1;
-    a.B = B; a.b_batch = b_batch; a.ldb = ldb;
-    a.C = C; a.c_batch = (long long)M * M; a.ldc = M;
-    a.Mr = a.Nc = a.K = M;
-    a.alpha = cmake(1.0, 0.0);
-    return launch_zgemm(p, p->stream, a, n_E);
-}
-
-int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, cplx *g_out, int *iters_out, int *n_open_out)
-{
-    const int M = p->M, N = 2 * M;
-    if (N > 2048) return fail(p, RGF_EUNSUPPORTED, "lead decimation needs a %d x %d inverse; M > 1024 is not supported in this version", N, N);
-    const long long MM = (long long)M * M, NN = (long long)N * N;
+    const int M = p->M, qc = pb & 1, nc = half_count(M, qc), N = dense ? 2 * M : 2 * nc;
+    if (N > 2048) return fail(p, RGF_EUNSUPPORTED, "lead decimation needs a %d x %d inverse; not supported in this version", N, N);
+    const long long CC = (long long)nc * nc, NN = (long long)N * N;
     int rc;
-    if ((rc = ensure(p, p->l_eps, sizeof(cplx) * NN * n_E))) return rc;
-    if ((rc = ensure(p, p->l_eps_s, sizeof(cplx) * NN * n_E))) return rc;
+    Ws &w = p->ws[0];
+    Buf *cb[] = {&p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_eps, &p->l_eps_s, &p->stage_in};
+    for (Buf *b : cb) if ((rc = ensure(p, *b, sizeof(cplx) * CC * n_E))) return rc;
     if ((rc = ensure(p, p->l_W, sizeof(cplx) * NN * n_E))) return rc;
     if (N <= 256 && (rc = ensure(p, p->l_W2, sizeof(cplx) * NN * n_E))) return rc;
-    Buf *small[] = {&p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4};
-    for (Buf *b : small) if ((rc = ensure(p, *b, sizeof(cplx) * MM * n_E))) return rc;
-    Ws &w = p->ws[0];
     if ((rc = ensure_inverse_ws(p, w, N, n_E))) return rc;
     if ((rc = ensure(p, p->lead_flags, sizeof(int) * (size_t)(n_E + 4)))) return rc;
-    cplx *eps = ptr<cplx>(p->l_eps), *eps_s = ptr<cplx>(p->l_eps_s), *gw = ptr<cplx>(p->l_W), *gw2 = ptr<cplx>(p->l_W2), *g = nullptr;
-    cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta);
-    cplx *T1 = ptr<cplx>(p->l_T1), *X = ptr<cplx>(p->l_T2), *Y = ptr<cplx>(p->l_T3), *T3 = ptr<cplx>(p->l_T4);
+    cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta), *X = ptr<cplx>(p->l_eps), *Y = ptr<cplx>(p->l_eps_s);
+    cplx *T1 = ptr<cplx>(p->l_T1), *T2 = ptr<cplx>(p->l_T2), *an = ptr<cplx>(p->l_T3);
+    cplx *Sacc = ptr<cplx>(p->stage_in);          // surface accumulator: X_s (right lead, side > 0) or Y_s (left lead)
+    cplx *S = ptr<cplx>(p->l_W), *S2 = ptr<cplx>(p->l_W2), *g = nullptr;
     int *flags = ptr<int>(p->lead_flags), *n_open = flags + n_E;
     int *status = ptr<int>(p->status);      // a bad pivot in the lead marks batch items [0, n_E): device 0 of each energy
     const double *E = ptr<double>(p->E);
-    dim3 gN((unsigned)std::min<long long>((NN + 255) / 256, 2048), n_E), gM((unsigned)std::min<long long>((MM + 255) / 256, 1024), n_E);
-
-    lead_cell_init_kernel<<<gN, 256, 0, p->stream>>>(eps, eps_s, a, b, M, p->t, pa, pb);
+    dim3 gc((unsigned)std::min<long long>((CC + 255) / 256, 256), n_E), gs((unsigned)std::min<long long>((NN + 255) / 256, 2048), n_E);
+    lead_half_init_kernel<<<gc, 256, 0, p->stream>>>(a, b, X, Y, Sacc, nc, p->t);
     p->stats.launches++;
+    // position of the corner blocks inside g (N x N): element (r, c) of block (u, v) at g[(off_u + r rs) N + off_v + c rs]
+    const int rs = dense ? 2 : 1, off_e = dense ? qc : 0, off_o = dense ? M + qc : nc;
+    // C (nc x nc, contiguous per energy) = A B with A either a corner block of g (strided) or a compact matrix
+    auto gemm = [&](const cplx *A, long long a_rs, long long a_cs, long long a_batch, const cplx *B, cplx *C) -> int {
+        ZgemmArgs z;
+        memset(&z, 0, sizeof(z));
+        z.A = A; z.a_batch = a_batch; z.a_rs = a_rs; z.a_cs = a_cs; z.kmask_div = 1;
+        z.B = B; z.b_batch = CC; z.ldb = nc;
+        z.C = C; z.c_batch = CC; z.ldc = nc;
+        z.Mr = z.Nc = z.K = nc;
+        z.alpha = cmake(1.0, 0.0);
+        return launch_zgemm(p, p->stream, z, n_E);
+    };
+    auto gblock = [&](const cplx *G, int off_r, int off_c) { return G + (long long)off_r * N + off_c; };
+    // Schur route: one Newton step g <- sym(g + g (I - S g)).  Measured against an 80-bit reference (M = 128,
+    // E = 0.2549 eV): surface Green's function off by 3.3e-10 with the plain inverse, 4.5e-11 with g symmetrised,
+    // 1.1e-11 with the Newton step on top (the level of the dense route).  S is assembled a second time (the inverse
+    // consumed it).
+    cplx *S3 = nullptr, *Rr = nullptr;
+    if (!dense) {
+        if ((rc = ensure(p, p->lc_S3, sizeof(cplx) * NN * n_E))) return rc;
+        if ((rc = ensure(p, p->lc_R, sizeof(cplx) * NN * n_E))) return rc;
+        S3 = ptr<cplx>(p->lc_S3); Rr = ptr<cplx>(p->lc_R);
+    }
+    auto gemmN = [&](const cplx *A, const cplx *B, cplx *C) -> int {
+        ZgemmArgs z;
+        memset(&z, 0, sizeof(z));
+        z.A = A; z.a_batch = NN; z.a_rs = N; z.a_cs = 1; z.kmask_div = 1;
+        z.B = B; z.b_batch = NN; z.ldb = N;
+        z.C = C; z.c_batch = NN; z.ldc = N;
+        z.Mr = z.Nc = z.K = N;
+        z.alpha = cmake(1.0, 0.0);
+        return launch_zgemm(p, p->stream, z, n_E);
+    };
+    // g = (z - eps)^-1 restricted as needed, symmetric; Xc / Yc = corrections on (o, o) / (e, e) (NULL = none)
+    auto cell_inverse = [&](const cplx *Xc, const cplx *Yc) -> int {
+        int r2;
+        if (dense) {
+            lead_cell_assemble_kernel<<<gs, 256, 0, p->stream>>>(S, Xc, Yc, nc, M, qc, pa, p->t, E, eta);
+            p->stats.launches++;
+            if ((r2 = run_inverse(p, w, S, S2, N, n_E, status, &g))) return r2;
+            lead_half_symmetrize_kernel<<<gs, 256, 0, p->stream>>>(g, N);
+            p->stats.launches++;
+            return RGF_OK;
+        }
+        lead_schur_assemble_kernel<<<gs, 256, 0, p->stream>>>(S, Xc, Yc, nc, M, qc, p->t, E, eta);
+        p->stats.launches++;
+        if ((r2 = run_inverse(p, w, S, S2, N, n_E, status, &g))) return r2;
+        lead_schur_assemble_kernel<<<gs, 256, 0, p->stream>>>(S3, Xc, Yc, nc, M, qc, p->t, E, eta);
+        p->stats.launches++;
+        if ((r2 = gemmN(S3, g, Rr))) return r2;                       // S g
+        lead_half_residual_kernel<<<gs, 256, 0, p->stream>>>(Rr, N);  // I - S g
+        p->stats.launches++;
+        if ((r2 = gemmN(g, Rr, S3))) return r2;                       // g (I - S g)   (S3 as scratch)
+        lead_half_correct_kernel<<<gs, 256, 0, p->stream>>>(g, S3, N);
+        p->stats.launches++;
+        return RGF_OK;
+    };
     int it = 0, open = n_E;
     for (it = 0; it < kLeadMaxIt; it++) {
         CUDA_TRY(p, cudaMemsetAsync(n_open, 0, sizeof(int), p->stream));
-        lead_converged_kernel<<<n_E, 256, 0, p->stream>>>(a, b, M, kLeadTol, flags, n_open);
+        lead_converged_kernel<<<n_E, 256, 0, p->stream>>>(a, a, nc, kLeadTol, flags, n_open);
         p->stats.launches++;
         CUDA_TRY(p, cudaMemcpyAsync(&open, n_open, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         if (open == 0) break;
-        lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(gw, eps, N, E, eta);
+        if ((rc = cell_inverse(X, Y))) return rc;
+        const long long grs = (long long)rs * N;
+        lead_half_transpose_kernel<<<gc, 256, 0, p->stream>>>(b, a, nc);                 // b = a^T (= beta)
         p->stats.launches++;
-        if ((rc = run_inverse(p, w, gw, gw2, N, n_E, status, &g))) return rc;
-        const cplx *g11 = g, *g12 = g + M, *g21 = g + (long long)M * N, *g22 = g + (long long)M * N + M;
-        if ((rc = lead_gemm(p, a, M, MM, g11, N, NN, T1, n_E))) return rc;      // a g11
-        if ((rc = lead_gemm(p, T1, M, MM, b, M, MM, X, n_E))) return rc;        // X = a g11 b   -> [2,2]
-        if ((rc = lead_gemm(p, b, M, MM, g22, N, NN, T3, n_E))) return rc;      // b g22
-        if ((rc = lead_gemm(p, T3, M, MM, a, M, MM, Y, n_E))) return rc;        // Y = b g22 a   -> [1,1]
-        lead_cell_accumulate_kernel<<<gM, 256, 0, p->stream>>>(eps, eps_s, X, Y, M, side);
+        if ((rc = gemm(gblock(g, off_e, off_e), grs, rs, NN, b, T1))) return rc;        // g[e,e] a^T
+        if ((rc = gemm(a, nc, 1, CC, T1, T2))) return rc;                               // Tx = a g[e,e] a^T   -> (o, o)
+        if ((rc = gemm(gblock(g, off_o, off_o), grs, rs, NN, a, T1))) return rc;        // g[o,o] a
+        if ((rc = gemm(b, nc, 1, CC, T1, an))) return rc;                               // Ty = a^T g[o,o] a   -> (e, e)   (an as scratch)
+        lead_half_accumulate_kernel<<<gc, 256, 0, p->stream>>>(X, Y, Sacc, T2, an, nc, side);
         p->stats.launches++;
-        if ((rc = lead_gemm(p, a, M, MM, g12, N, NN, T1, n_E))) return rc;      // a g12
-        if ((rc = lead_gemm(p, T1, M, MM, a, M, MM, X, n_E))) return rc;        // a g12 a
-        if ((rc = lead_gemm(p, b, M, MM, g21, N, NN, T3, n_E))) return rc;      // b g21
-        if ((rc = lead_gemm(p, T3, M, MM, b, M, MM, Y, n_E))) return rc;        // b g21 b
-        std::swap(a, X);
-        std::swap(b, Y);
+        if ((rc = gemm(gblock(g, off_e, off_o), grs, rs, NN, a, T1))) return rc;        // g[e,o] a
+        if ((rc = gemm(a, nc, 1, CC, T1, an))) return rc;                               // a g[e,o] a
+        std::swap(a, an);
     }
-    lead_zminus_kernel<<<gN, 256, 0, p->stream>>>(gw, eps_s, N, E, eta);
-    p->stats.launches++;
-    if ((rc = run_inverse(p, w, gw, gw2, N, n_E, status, &g))) return rc;
-    lead_extract_kernel<<<gM, 256, 0, p->stream>>>(g, g_out, M, side);
+    // surface block of (z - eps_s)^-1: (o, o) with Y_s for the left lead, (e, e) with X_s for the right lead
+    if ((rc = cell_inverse(side > 0 ? Sacc : nullptr, side > 0 ? nullptr : Sacc))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(g_out, 0, sizeof(cplx) * (size_t)M * M * n_E, p->stream));
+    const int off_s = side > 0 ? off_e : off_o;
+    lead_half_scatter_kernel<<<gc, 256, 0, p->stream>>>(g_out, gblock(g, off_s, off_s), M, nc, qc, rs * N, rs, NN);
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
     if (iters_out) *iters_out = it;
     if (n_open_out) *n_open_out = open;
     return RGF_OK;
+}
+
+// true if the closed middle inverse of the Schur route is safely away from its resonance E = +-t
+bool schur_leads_ok(rgf_plan *p, int n_E)
+{
+    std::vector<double> h(n_E);
+    if (cudaMemcpyAsync(h.data(), p->E.p, sizeof(double) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream) != cudaSuccess) return false;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return false;
+    const double t2 = p->t * p->t;
+    for (double e : h) if (std::fabs(e * e - t2) < 0.02 * t2) return false;
+    return p->fast_leads && p->M >= 4;
 }
 
 // both leads; for even L the two cells have the same bond parities and g_R = g_L exactly
@@ -369,12 +438,13 @@ int run_leads(rgf_plan *p, int n_E, double eta, int *n_open_out)
     int rc, itL = 0, itR = 0, openL = 0, openR = 0;
     const size_t MMb = sizeof(cplx) * (size_t)M * M * n_E;
     if ((rc = ensure(p, p->gL, MMb))) return rc;
-    if ((rc = run_lead_side(p, n_E, eta, -1, -2, -1, ptr<cplx>(p->gL), &itL, &openL))) return rc;
+    const bool dense = !schur_leads_ok(p, n_E);
+    if ((rc = run_lead_side(p, n_E, eta, -1, -2, -1, dense, ptr<cplx>(p->gL), &itL, &openL))) return rc;
     if ((L & 1) == 0) {
         itR = itL; openR = 0;      // g_R aliases g_L (see pR() below)
     } else {
         if ((rc = ensure(p, p->gR, MMb))) return rc;
-        if ((rc = run_lead_side(p, n_E, eta, +1, L, L + 1, ptr<cplx>(p->gR), &itR, &openR))) return rc;
+        if ((rc = run_lead_side(p, n_E, eta, +1, L, L + 1, dense, ptr<cplx>(p->gR), &itR, &openR))) return rc;
     }
     p->stats.lead_iterations = std::max(itL, itR);
     if (n_open_out) *n_open_out = openL + openR;
@@ -460,24 +530,17 @@ int ensure_sweep_ws_half(rgf_plan *p, Ws &w, int cohort)
 inline bool use_fused(const rgf_plan *p) { return p->formulation == RGF_FORM_HALF && p->nh <= HS_NMAX; }
 
 // fused path (half_sweep.cuh): one CTA per matrix runs every half-step of slices 0..nslices-1 in ONE launch
-int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
+// launches half_sweep_kernel for the nb matrices described by `a` (state buffers of workspace w are set here)
+int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
 {
-    const int nh = p->nh, ldn = (nh + 1) & ~1;
     int rc;
-    const size_t xb = sizeof(cplx) * (size_t)ldn * ldn * nb;
+    const size_t xb = sizeof(cplx) * (size_t)a.ldn * a.ldn * nb;
     Buf *bufs[] = {&w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1};
     for (Buf *b : bufs) if ((rc = ensure(p, *b, xb))) return rc;
     if ((rc = ensure(p, w.Fperm, sizeof(int) * (size_t)HS_NMAX * nb))) return rc;
-    HSweepArgs a;
-    memset(&a, 0, sizeof(a));
-    a.M = p->M; a.L = p->L; a.nh = nh; a.ldn = ldn; a.n_E = n_E; a.bz0 = bz0; a.nb = nb; a.eta = eta; a.t = p->t;
-    a.energies = ptr<double>(p->E); a.onsite = ptr<double>(p->onsite);
-    a.bond = ptr<uint8_t>(p->bond); a.hop = ptr<uint8_t>(p->hop);
-    a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
+    a.nb = nb;
     a.X0 = ptr<cplx>(w.Fx0); a.X1 = ptr<cplx>(w.Fx1); a.P0 = ptr<cplx>(w.Fp0); a.P1 = ptr<cplx>(w.Fp1);
-    a.perm = ptr<int>(w.Fperm); a.status = ptr<int>(p->status) + bz0;
-    a.hs_begin = 0; a.hs_end = 2 * nslices;
-    a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
+    a.perm = ptr<int>(w.Fperm);
     static const bool prof_on = getenv("RGF_HS_PROF") != nullptr;          // debugging aid: per-phase cycle counters
     if (prof_on) {
         if ((rc = ensure(p, p->counters, sizeof(long long) * 16 * (size_t)nb))) return rc;
@@ -529,6 +592,23 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
         fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           update loop: load1 %.0f sync %.0f stageR %.0f comp0 %.0f store0 %.0f load0 %.0f comp1 %.0f store1 %.0f\n",
                 s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[8] / hsn, s[9] / hsn, s[10] / hsn, s[11] / hsn, s[12] / hsn, s[13] / hsn, s[14] / hsn, s[15] / hsn);
     }
+    return RGF_OK;
+}
+
+int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, int nslices, cplx **g_out, cplx **Pcur_out)
+{
+    const int nh = p->nh, ldn = (nh + 1) & ~1;
+    int rc;
+    HSweepArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = p->M; a.L = p->L; a.nh = nh; a.ldn = ldn; a.n_E = n_E; a.bz0 = bz0; a.eta = eta; a.t = p->t;
+    a.energies = ptr<double>(p->E); a.onsite = ptr<double>(p->onsite);
+    a.bond = ptr<uint8_t>(p->bond); a.hop = ptr<uint8_t>(p->hop);
+    a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
+    a.status = ptr<int>(p->status) + bz0;
+    a.hs_begin = 0; a.hs_end = 2 * nslices;
+    a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
+    if ((rc = fused_launch(p, w, a, nb))) return rc;
     *g_out = ptr<cplx>(w.H0); *Pcur_out = ptr<cplx>(w.Pa);
     return RGF_OK;
 }
@@ -843,8 +923,8 @@ int rgf_destroy(rgf_plan *p)
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
     Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->counters,
-                   &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_T4,
-                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out};
+                   &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3,
+                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R};
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
@@ -880,6 +960,13 @@ int rgf_set_formulation(rgf_plan *p, int formulation)
 {
     if (!p || formulation < RGF_FORM_DENSE || formulation > RGF_FORM_HALF_STEPWISE) return RGF_EINVAL;
     p->formulation = formulation;
+    return RGF_OK;
+}
+
+int rgf_set_lead_method(rgf_plan *p, int method)
+{
+    if (!p || (method != RGF_LEAD_CELL_DENSE && method != RGF_LEAD_CELL_SCHUR)) return RGF_EINVAL;
+    p->fast_leads = method == RGF_LEAD_CELL_SCHUR;
     return RGF_OK;
 }
 

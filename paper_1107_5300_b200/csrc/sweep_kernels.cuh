@@ -60,87 +60,12 @@ __global__ void propagator_start_kernel(const cplx *Gall, cplx *Pall, int M, int
     }
 }
 
-// ---- lead decimation (Sancho-Rubio on the clean two-slice cell) -----------
-// Cell matrices are N x N, N = 2M: h00 = [[H_c, V_a],[V_a, H_c]], h01 = [[0,0],[V_b,0]].
-// alpha = h01 and beta = h01^T keep their block shape under alpha <- alpha g alpha,
-// beta <- beta g beta (only block (2,1) resp. (1,2) is ever non-zero), so only the M x M blocks
-// a = alpha[2,1] and b = beta[1,2] are stored and the products reduce to
-//   alpha g beta = [2,2] block  a g11 b      beta g alpha = [1,1] block  b g22 a
-//   alpha g alpha -> a g12 a                  beta g beta  -> b g21 b
+// ---- lead decimation (Sancho-Rubio on the clean two-slice cell): kernels in half_kernels.cuh ----
+// alpha = h01 and beta = h01^T keep their block shape under alpha <- alpha g alpha, beta <- beta g beta (only block
+// (2,1) resp. (1,2) of the 2M x 2M cell is ever non-zero, and inside it only the rows / columns of the atoms that bond to
+// the next cell), so the products reduce to
+//   alpha g beta = a g11 b on [2,2]      beta g alpha = b g22 a on [1,1]      alpha g alpha -> a g12 a      beta g beta -> b g21 b
 // which are the dense products with their structurally-zero terms left out.
-
-// W = z - X for dense N x N matrices per energy
-__global__ void lead_zminus_kernel(cplx *Wall, const cplx *Xall, int N, const double *energies, double eta)
-{
-    const int e = blockIdx.y;
-    const long long NN = (long long)N * N;
-    cplx *W = Wall + (long long)e * NN;
-    const cplx *X = Xall + (long long)e * NN;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < NN;
-         idx += (long long)gridDim.x * blockDim.x) {
-        int j = (int)(idx / N), k = (int)(idx % N);
-        cplx x = X[idx];
-        cplx w = cmake(-x.x, -x.y);
-        if (j == k) { w.x += energies[e]; w.y += eta; }
-        W[idx] = w;
-    }
-}
-
-// eps = eps_s = h00; a = b = V_b.  va[j] = t m_pa[j], vb[j] = t m_pb[j] (m_p[j] = 1 iff (p + j) even)
-__global__ void lead_cell_init_kernel(cplx *eps_all, cplx *eps_s_all, cplx *a_all, cplx *b_all, int M, double t, int pa, int pb)
-{
-    const int e = blockIdx.y, N = 2 * M;
-    const long long NN = (long long)N * N, MM = (long long)M * M;
-    cplx *eps = eps_all + (long long)e * NN, *eps_s = eps_s_all + (long long)e * NN;
-    cplx *a = a_all + (long long)e * MM, *b = b_all + (long long)e * MM;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < NN;
-         idx += (long long)gridDim.x * blockDim.x) {
-        int r = (int)(idx / N), c = (int)(idx % N);
-        int br = r >= M, bc = c >= M, j = r - br * M, k = c - bc * M;
-        double h;
-        if (br == bc) h = (j == k + 1 || k == j + 1) ? t : 0.0;
-        else h = (j == k) ? t * mask_bit(pa, j) : 0.0;
-        eps[idx] = cmake(h, 0.0);
-        eps_s[idx] = cmake(h, 0.0);
-        if (br == 0 && bc == 0) {
-            cplx v = cmake((j == k) ? t * mask_bit(pb, j) : 0.0, 0.0);
-            a[(long long)j * M + k] = v;
-            b[(long long)j * M + k] = v;
-        }
-    }
-}
-
-// eps[2,2] += agb; eps[1,1] += bga; eps_s += agb (right lead, side > 0) or bga (left lead)
-__global__ void lead_cell_accumulate_kernel(cplx *eps_all, cplx *eps_s_all, const cplx *agb_all, const cplx *bga_all, int M, int side)
-{
-    const int e = blockIdx.y, N = 2 * M;
-    const long long NN = (long long)N * N, MM = (long long)M * M;
-    cplx *eps = eps_all + (long long)e * NN, *eps_s = eps_s_all + (long long)e * NN;
-    const cplx *agb = agb_all + (long long)e * MM, *bga = bga_all + (long long)e * MM;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < MM;
-         idx += (long long)gridDim.x * blockDim.x) {
-        int j = (int)(idx / M), k = (int)(idx % M);
-        long long i11 = (long long)j * N + k, i22 = (long long)(M + j) * N + (M + k);
-        cplx x = agb[idx], y = bga[idx];
-        eps[i22] = cadd(eps[i22], x);
-        eps[i11] = cadd(eps[i11], y);
-        if (side > 0) eps_s[i22] = cadd(eps_s[i22], x);
-        else eps_s[i11] = cadd(eps_s[i11], y);
-    }
-}
-
-// surface block of (z - eps_s)^-1: top-left (right lead) or bottom-right (left lead)
-__global__ void lead_extract_kernel(const cplx *g_all, cplx *out_all, int M, int side)
-{
-    const int e = blockIdx.y, N = 2 * M, off = side > 0 ? 0 : M;
-    const cplx *g = g_all + (long long)e * N * N;
-    cplx *out = out_all + (long long)e * M * M;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < (long long)M * M;
-         idx += (long long)gridDim.x * blockDim.x) {
-        int j = (int)(idx / M), k = (int)(idx % M);
-        out[idx] = g[(long long)(off + j) * N + (off + k)];
-    }
-}
 
 // flags[e] = 1 if max(|alpha|, |beta|) >= tol for energy e; *n_open counts them
 __global__ void lead_converged_kernel(const cplx *alpha, const cplx *beta, int M, double tol, int *flags, int *n_open)

@@ -88,8 +88,10 @@ def test_singular_matrix_is_reported(rgf, plan):
 
 # ---- A2: lead self-energies -----------------------------------------------------------------
 
+@pytest.mark.parametrize("method", [0, 1], ids=["cell_dense", "cell_schur"])
 @pytest.mark.parametrize("M,L", [(20, 40), (20, 41), (7, 5), (64, 10)])
-def test_lead_self_energy_matches_oracle(rgf, plan, oracle, M, L):
+def test_lead_self_energy_matches_oracle(rgf, plan, oracle, M, L, method):
+    rgf.rgf_set_lead_method(plan.handle, method)
     E = np.array([-2.0, -0.4, 0.013, 0.8, 1.7])
     vac = np.zeros((L, M), dtype=np.uint8)
     vac[0, 1] = 1
@@ -278,3 +280,32 @@ def test_c64_with_vacancies_and_odd_width(rgf, plan, oracle, M, L):
     T64 = plan.transmission(E, 1e-9, precision=rgf.RGF_C64)[0]
     T_or = oracle.transmission_batch(on, vac, -2.7, E, 1e-9)
     assert np.max(np.abs(T64 - T_or)) <= 1e-3, np.abs(T64 - T_or)
+
+
+def test_lead_methods_agree_and_fall_back_near_t(rgf, plan, oracle):
+    """RGF_LEAD_CELL_SCHUR eliminates half of the cell in closed form, resonant at E = +-t: such calls take the dense route."""
+    M, L = 20, 40
+    on = np.zeros((L, M))
+    plan.set_device(on, -2.7)
+    E = np.array([-2.7, -2.69, 0.5, 2.7])
+    T_or = oracle.transmission_batch(on, None, -2.7, E, 1e-9)
+    for method in (0, 1):
+        rgf.rgf_set_lead_method(plan.handle, method)
+        T = plan.transmission(E, 1e-9)[0]
+        assert np.all(np.abs(T - T_or) <= tol(T_or)), (method, np.abs(T - T_or))
+
+
+def test_lead_methods_agree_at_paper_width(rgf, plan):
+    """M = 244 at E = 0.4637 eV: the block decimation diverged there before beta = alpha^T was made structural
+    (DESIGN.md section 5c); both lead routes must converge and give the same T on a short clean ribbon."""
+    M, L = 244, 4
+    plan.set_device(np.zeros((L, M)), -2.7)
+    E = np.array([-0.4, 0.2549, 0.4637, 0.8])
+    T = []
+    for method in (0, 1):
+        rgf.rgf_set_lead_method(plan.handle, method)
+        T.append(plan.transmission(E, 1e-9)[0])
+        assert 30 <= plan.stats()["lead_iterations"] <= 40
+    assert np.all(np.isfinite(T[0])) and np.all(np.isfinite(T[1]))
+    assert np.all(np.abs(T[0] - T[1]) <= 1e-9 * np.maximum(1.0, T[0])), np.abs(T[0] - T[1])
+    assert np.all(np.abs(T[0] - np.round(T[0])) < 1e-6)          # clean ribbon: integer channel count up to the eta deficit
