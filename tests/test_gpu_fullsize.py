@@ -124,3 +124,22 @@ def test_config3_c64_vs_c128(plan, disordered):
         assert np.quantile(d[outside], 0.90) <= 1e-3, np.quantile(d[outside], 0.90)
         assert np.all(d[outside] <= 1e-3 + 5e-5 * T128[outside]), (d[outside] / T128[outside]).max()
     assert d.max() > 1e-9          # a different precision really ran
+
+
+def test_config4_wide_ribbon_full_length_properties(plan):
+    """configs[4] at full size (M = 1024, L = 2000, 64 energies, edge vacancies): no oracle value exists at this length
+    (hours per energy), so the properties that hold at any size are checked: finite, 0 <= T <= open lead channels,
+    and the same T from the dense formulation on a sub-sample of energies."""
+    from paper_1107_5300_b200 import binding as rgf
+    w = inputs.config4()
+    plan.set_device(w.onsite, w.t, w.vacancy)
+    T = plan.transmission(w.energies, w.eta)
+    assert T.shape == (1, 64) and np.all(np.isfinite(T))
+    nch = np.array([n_open_channels(w.M, e) for e in w.energies])
+    assert np.all(T >= -1e-9) and np.all(T[0] <= nch + 1e-8), (T.min(), (T[0] - nch).max())
+    st = plan.stats()
+    print("configs[4] full length: %.1f s (leads %.1f s), %d launches" % (st["ms_total"] / 1e3, st["ms_leads"] / 1e3, st["launches"]))
+    sub = np.array([3, 31, 60])
+    rgf.rgf_set_formulation(plan.handle, rgf.RGF_FORM_DENSE)
+    Td = plan.transmission(w.energies[sub], w.eta)[0]
+    assert np.all(np.abs(Td - T[0, sub]) <= 1e-9 * np.maximum(1.0, Td)), np.abs(Td - T[0, sub])
