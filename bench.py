@@ -36,7 +36,7 @@ from paper_1107_5300_b200 import inputs  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the headline launch configuration,
 # from the ncu --set full capture summarised in profiles/ (bytes; None = not captured for this formulation)
-TRAFFIC_NCU = {"half": 84.75e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
+TRAFFIC_NCU = {"half": 84.33e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
 
 METRIC = "rgf_slice_steps_per_s"
 UNIT = "slice-steps/s"
