@@ -26,7 +26,10 @@ namespace rgf {
 constexpr int HS_NT = 256, HS_NMAX = 128, HS_B = 32, HS_SB = 8;
 constexpr int HS_LDP = HS_B + 4;        // 36: A-fragment reads of the panel conflict-free
 constexpr int HS_LDR = HS_B + 2;        // 34: B-fragment reads conflict-free
-constexpr int HS_STAGE_ROWS = 36;       // the panel buffer seen as rows of HS_NMAX elements (assembly staging)
+constexpr int HS_STAGE_ROWS = 36;
+#ifndef HS_RG
+#define HS_RG 2                         // row blocks of 8 per register tile of the strip update
+#endif       // the panel buffer seen as rows of HS_NMAX elements (assembly staging)
 
 struct HSweepArgs {
     int M, L, nh, ldn, n_E, bz0, nb;
@@ -41,6 +44,7 @@ struct HSweepArgs {
     int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
                                   // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
     long long *prof;              // optional [nb][16] cycle counters of thread 0 per phase (NULL = off)
+    int stagger;                  // cycles the second CTA to arrive on an SM waits before its first half-step (see the kernel)
     cplx *g_out, *P_out;          // after half-step hs_end - 1: g dense n x n (ld n) and P (ld nh), stride nh*nh; may be NULL
 };
 
@@ -381,7 +385,112 @@ __device__ __forceinline__ void hs_half_store(const HSHalf &h, cplx *Cg, int ld,
     }
 }
 
+// ---- barrier-free update of one 8-column strip: C[:, col0 .. col0+8) += Mult (n x 32, sm.panel) * R ---------------
+// R = the strip's 32 pivot rows, snapshotted into the warp's B fragments (registers) before any row of the strip is
+// written, so a warp needs nothing from the other warps: no R staging through shared memory, no barrier per chunk, and
+// the warps drift apart so that one warp's loads / stores overlap another's DMMAs.  Row groups of 8 RG rows; the next
+// group's C fragments are in flight from L2 while the current group is on the tensor pipe.
+template <int RG>
+struct HSAcc { double re[RG][2], im[RG][2]; };
+
+template <int RG>
+__device__ __forceinline__ void hs_acc_load(HSAcc<RG> &h, const cplx *Cg, int ld, int n, int r0, bool cok)
+{
+    const int lane = threadIdx.x & 31, g = lane >> 2;
+#pragma unroll
+    for (int i = 0; i < RG; i++) {
+        const int rr = r0 + i * 8 + g;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        if (rr < n && cok) ld256cg(Cg + (long long)rr * ld, a0, a1, a2, a3);
+        h.re[i][0] = a0; h.im[i][0] = a1; h.re[i][1] = a2; h.im[i][1] = a3;
+    }
+}
+template <int RG>
+__device__ __forceinline__ void hs_acc_store(const HSAcc<RG> &h, cplx *Cg, int ld, int n, int r0, bool cok)
+{
+    const int lane = threadIdx.x & 31, g = lane >> 2;
+#pragma unroll
+    for (int i = 0; i < RG; i++) {
+        const int rr = r0 + i * 8 + g;
+        if (rr < n && cok) st256(Cg + (long long)rr * ld, h.re[i][0], h.im[i][0], h.re[i][1], h.im[i][1]);
+    }
+}
+template <int RG, bool FULL>
+__device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, int r0, const cplx (&bb)[8], int kq)
+{
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const cplx *cA = panel + (r0 + g) * HS_LDP + t;
+    if (FULL) {
+        // straight-line code for a full 32-column panel: the A fragments of step q + 1 are loaded before the DMMAs of step q
+        cplx a[2][RG];
+#pragma unroll
+        for (int i = 0; i < RG; i++) a[0][i] = cA[i * 8 * HS_LDP];
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            if (q + 1 < 8) {
+#pragma unroll
+                for (int i = 0; i < RG; i++) a[(q + 1) & 1][i] = cA[i * 8 * HS_LDP + (q + 1) * 4];
+            }
+#ifndef HS_DIAG_NOMMA
+#pragma unroll
+            for (int i = 0; i < RG; i++) zmma884(h.re[i], h.im[i], a[q & 1][i].x, a[q & 1][i].y, -a[q & 1][i].y, bb[q].x, bb[q].y);
+#else
+#pragma unroll
+            for (int i = 0; i < RG; i++) { h.re[i][0] += a[q & 1][i].x * bb[q].x; h.im[i][1] += a[q & 1][i].y * bb[q].y; }
+#endif
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            if (q < kq) {
+                cplx a[RG];
+#pragma unroll
+                for (int i = 0; i < RG; i++) a[i] = cA[i * 8 * HS_LDP + q * 4];
+#pragma unroll
+                for (int i = 0; i < RG; i++) zmma884(h.re[i], h.im[i], a[i].x, a[i].y, -a[i].y, bb[q].x, bb[q].y);
+            }
+        }
+    }
+}
+
+template <int RG, bool FULL>
+__device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw)
+{
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    cplx bb[8];
+    {
+        const bool colok = col0 + g < ncols;
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            const int k = q * 4 + t;
+            bb[q] = cmake(0.0, 0.0);
+            if (k < bw && colok) bb[q] = ldcg(Cg + (long long)prow[k] * ld + col0 + g);
+        }
+    }
+    const int kq = (bw + 3) >> 2;
+#ifdef HS_DIAG_NOMEM
+    const bool cok = false;
+#else
+    const bool cok = col0 + 2 * t < ncols;
+#endif
+    cplx *Cl = Cg + col0 + 2 * t;
+    constexpr int GR = 8 * RG;
+    HSAcc<RG> h0, h1;
+    hs_acc_load<RG>(h0, Cl, ld, n, 0, cok);
+    for (int r0 = 0; r0 < n; r0 += 2 * GR) {
+        hs_acc_load<RG>(h1, Cl, ld, n, r0 + GR, cok);
+        hs_acc_compute<RG, FULL>(h0, panel, r0, bb, kq);
+        hs_acc_store<RG>(h0, Cl, ld, n, r0, cok);
+        hs_acc_load<RG>(h0, Cl, ld, n, r0 + 2 * GR, cok);
+        if (r0 + GR < n) {
+            hs_acc_compute<RG, FULL>(h1, panel, r0 + GR, bb, kq);
+            hs_acc_store<RG>(h1, Cl, ld, n, r0 + GR, cok);
+        }
+    }
+}
+
 // ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry); fills sm.perm / sm.pinv ------------------------
+template <int MODE>
 __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof)
 {
     long long tc = prof ? clock64() : 0;
@@ -411,6 +520,24 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         }
         __syncthreads();
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
+        if constexpr (MODE == 1) {
+            // strip list: the 8-column strips of X except the panel's own four, then the strips of W; warp w takes
+            // strips w, w + 8, ...
+            __syncthreads();
+            HS_TICK(3);
+            const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3, sk0 = k0 >> 3;
+            const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;
+            const int nxs = nsx - (sk1 - sk0), tot = nxs + nsw;
+            for (int s = tid >> 5; s < tot; s += HS_NT / 32) {
+                cplx *Cg = W; int col0 = (s - nxs) * 8, ncols = nc;
+                if (s < nxs) { Cg = X; col0 = (s < sk0 ? s : s + (sk1 - sk0)) * 8; ncols = n; }
+                if (bw == HS_B) hs_strip_update<HS_RG, true>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw);
+                else hs_strip_update<HS_RG, false>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw);
+            }
+            __syncthreads();
+            HS_TICK(4);
+            continue;
+        }
         // chunk list: matrix chunks except the panel's own, then the propagator chunks
         const int skip = k0 / HS_B, total = nchm - 1 + ncha;
         const int kmax = (bw + 3) & ~3;
@@ -453,8 +580,13 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
 // ---- assembly of A (into Xn) and of W = C P_prev (into Wn) for half-step (i, kind) -------------------------
 // g_prev[k][m] = Xp[perm_prev[k]][pinv_prev[m]], P_prev[k][:] = Wp[perm_prev[k]][:]; blocks of 32 output rows,
 // the physical rows they need staged in the (idle) panel buffer so that every L2 read is a full row.
-template <class SM, int NT>
-__device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl, int i, int kind, bool first,
+struct HSAsm {
+    cplx *stage;                       // staging area of 2 (RB + 2) rows of HS_NMAX elements (the idle panel buffer)
+    HSTab *tb;                         // per-row tables (alias the idle candidate buffers)
+    const int *perm_prev, *pinv_prev;  // row maps of the previous half-step
+};
+template <int NT, int RB>
+__device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a, int bl, int i, int kind, bool first,
                                             const cplx *Xp, const cplx *Wp, cplx *Xn, cplx *Wn)
 {
     constexpr int HS_NT = NT;        // threads that run the assembly (the whole CTA of either kernel)
@@ -468,7 +600,7 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
     const uint8_t *mk = a.bond + ((long long)d * (L + 1) + i) * M;        // m'_{i-1}
     const uint8_t *mr = a.bond + ((long long)d * (L + 1) + L) * M;        // m'_{L-1}
     const uint8_t *hp = a.hop + ((long long)d * L + i) * M;
-    cplx *stage = sm.panel;                                                // [<= 36][HS_NMAX]
+    cplx *stage = sm.stage;
     if (first) {
         // half-step 0 (B_0): g_prev = surface Green's function of the left lead (slice -1, same atoms j), W = I
         const cplx *gl = a.gL + (long long)e * MM;
@@ -490,7 +622,7 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
     // per-row tables of this half-step (the candidate buffers of the pivot search are idle here):
     //   kind B: ra[r] = m'[r];                       ca[c] = m'[c] ? physical column of g_prev[.][c] : -1
     //   kind F: ra/rb[r] = lower / upper B neighbour; ca/cb[c] = physical column of that neighbour, or -1
-    HSTab &tb = *reinterpret_cast<HSTab *>(sm.crow);
+    HSTab &tb = *sm.tb;
     if (tid < n) {
         const int r = tid;
         tb.eps[r] = E - eps[2 * r + par];
@@ -508,8 +640,7 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
     __syncthreads();
     // blocks of 16 output rows; the (<= 18) physical rows a block needs are staged by cp.async into one of two areas of
     // the panel buffer, the next block's rows in flight while this block is computed
-    constexpr int RB = 16, AREA = (RB + 2) * HS_NMAX;
-    static_assert(2 * AREA <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
+    constexpr int AREA = (RB + 2) * HS_NMAX;
     auto rows_of = [&](int r0, int &slo, int &nst) {
         const int r1 = (r0 + RB < n) ? r0 + RB : n;
         int shi = r1 - 1;
@@ -598,7 +729,10 @@ __device__ __forceinline__ void hs_assemble(SM &sm, const HSweepArgs &a, int bl,
     __syncthreads();          // the tables alias the pivot-search buffers
 }
 
+__device__ unsigned hs_sm_arrivals[256];
+
 // ---- the sweep: one CTA per matrix, half-steps [hs_begin, hs_end) ----------------------------------------
+template <int MODE>
 __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
 {
     extern __shared__ __align__(16) unsigned char hs_smem_raw[];
@@ -609,6 +743,21 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
     const int hs_begin = a.hs_begin + (int)(unit / a.nb) * a.unit_len;
     const int hs_end = (hs_begin + a.unit_len < a.hs_end) ? hs_begin + a.unit_len : a.hs_end;
     if (hs_begin >= hs_end) return;
+    // The two CTAs of an SM start a launch together and do identical work, so their phases (assembly / panel
+    // factorisation = FP64 pipe nearly idle, updates = FP64 tensor pipe saturated) stay aligned and nothing overlaps.
+    // Every second CTA to arrive on an SM therefore waits `stagger` cycles (about half a panel period) once per launch.
+    if (a.stagger > 0) {
+        if (tid == 0) {
+            unsigned smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            const unsigned arrival = atomicAdd(&hs_sm_arrivals[smid & 255], 1u);
+            if (arrival & 1u) {
+                const long long t0 = clock64();
+                while (clock64() - t0 < a.stagger) __nanosleep(200);
+            }
+        }
+        __syncthreads();
+    }
     const long long xs = (long long)ld * ld;
     cplx *Xb[2] = {a.X0 + bl * xs, a.X1 + bl * xs};
     cplx *Wb[2] = {a.P0 + bl * xs, a.P1 + bl * xs};
@@ -629,11 +778,13 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         if (tid < HS_NMAX) { sm.perm_prev[tid] = sm.perm[tid]; sm.pinv_prev[tid] = sm.pinv[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
-        hs_assemble<HSmem, 256>(sm, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
+        static_assert(2 * (16 + 2) * HS_NMAX <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
+        const HSAsm av = {sm.panel, reinterpret_cast<HSTab *>(sm.crow), sm.perm_prev, sm.pinv_prev};
+        hs_assemble<HS_NT, 16>(av, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
         __syncthreads();
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         n = half_count(M, kind == 0 ? ((i + 1) & 1) : (i & 1));
-        hs_gauss_jordan(sm, Xb[cur ^ 1], Wb[cur ^ 1], ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr);
+        hs_gauss_jordan<MODE>(sm, Xb[cur ^ 1], Wb[cur ^ 1], ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr);
     }
     if (tid < HS_NMAX) gperm[tid] = sm.perm[tid];
     if (a.prof && tid < 16) a.prof[bl * 16 + tid] += sm.prof[tid];
