@@ -27,6 +27,9 @@ constexpr int HS_NT = 256, HS_NMAX = 128, HS_B = 32, HS_SB = 8;
 constexpr int HS_LDP = HS_B + 4;        // 36: A-fragment reads of the panel conflict-free
 constexpr int HS_LDR = HS_B + 2;        // 34: B-fragment reads conflict-free
 constexpr int HS_STAGE_ROWS = 36;
+#ifndef HS_FSB
+#define HS_FSB 8                        // sub-block width of the panel factorisation
+#endif
 #ifndef HS_RG
 #define HS_RG 2                         // row blocks of 8 per register tile of the strip update
 #endif       // the panel buffer seen as rows of HS_NMAX elements (assembly staging)
@@ -131,11 +134,11 @@ struct HSGroup {
 // 12 mantissa bits: any pivot within 2^-12 of the largest magnitude is as good as the maximum) and 255 - row,
 // so the key is unique, names the row, and the lowest row wins ties.  The pivot row is not a divergent branch:
 //   row[j] <- c + a * pivrow[j]   with (a, c) = (d, 0) on the pivot row and (-x d, row[j]) elsewhere, row[CC] <- a.
-template <int CC>
-__device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &gr, cplx (&row)[HS_SB], bool &used, int kglob, int *status_slot)
+template <int CC, int SB>
+__device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &gr, cplx (&row)[SB], bool &used, int kglob, int *status_slot)
 {
     const int r = gr.r, warp = gr.slot, naw = gr.nslots;
-    constexpr int SB = HS_SB, NW = HS_NT / 32;
+    constexpr int NW = HS_NT / 32;
     constexpr int pb = (CC & 1) * NW;
 #ifdef HS_DBG
     long long td0 = clock64();
@@ -204,9 +207,13 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
 // ---- panel factorisation in shared memory: columns [k0, k0 + bw) of all n rows --------------------
 // On entry sm.panel[r][c] = X[r][k0 + c] (zero for c >= bw, r >= n).  On exit sm.panel = N' (the
 // transformed columns), sm.prow[c] = pivot row of column k0 + c, perm / pinv updated, used |= pivot.
+// SB = columns per register sub-block: 8 (two DMMA k-steps per in-panel update) or 4 (one k-step; half the FP64
+// instructions per pivot step, which is what counts when the pivot chain runs beside another warp's DMMAs)
+template <int SB = HS_SB>
 __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup &gr, int n, int k0, int bw, bool &used, int *status_slot)
 {
-    constexpr int B = HS_B, SB = HS_SB, LDP = HS_LDP, LDR = HS_LDR;
+    constexpr int B = HS_B, LDP = HS_LDP, LDR = HS_LDR;
+    static_assert(SB == 8 || SB == 4, "sub-block width");
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int r = gr.r;
     const bool has_row = r < n;
@@ -228,14 +235,16 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
         }
         if (gr.slot < gr.nslots) {
             const int kg = k0 + c0;
-            hs_pivot_step<0>(sm, gr, row, used, kg, status_slot);
-            if (ncols > 1) hs_pivot_step<1>(sm, gr, row, used, kg + 1, status_slot);
-            if (ncols > 2) hs_pivot_step<2>(sm, gr, row, used, kg + 2, status_slot);
-            if (ncols > 3) hs_pivot_step<3>(sm, gr, row, used, kg + 3, status_slot);
-            if (ncols > 4) hs_pivot_step<4>(sm, gr, row, used, kg + 4, status_slot);
-            if (ncols > 5) hs_pivot_step<5>(sm, gr, row, used, kg + 5, status_slot);
-            if (ncols > 6) hs_pivot_step<6>(sm, gr, row, used, kg + 6, status_slot);
-            if (ncols > 7) hs_pivot_step<7>(sm, gr, row, used, kg + 7, status_slot);
+            hs_pivot_step<0, SB>(sm, gr, row, used, kg, status_slot);
+            if (ncols > 1) hs_pivot_step<1, SB>(sm, gr, row, used, kg + 1, status_slot);
+            if (ncols > 2) hs_pivot_step<2, SB>(sm, gr, row, used, kg + 2, status_slot);
+            if (ncols > 3) hs_pivot_step<3, SB>(sm, gr, row, used, kg + 3, status_slot);
+            if constexpr (SB == 8) {
+                if (ncols > 4) hs_pivot_step<4, SB>(sm, gr, row, used, kg + 4, status_slot);
+                if (ncols > 5) hs_pivot_step<5, SB>(sm, gr, row, used, kg + 5, status_slot);
+                if (ncols > 6) hs_pivot_step<6, SB>(sm, gr, row, used, kg + 6, status_slot);
+                if (ncols > 7) hs_pivot_step<7, SB>(sm, gr, row, used, kg + 7, status_slot);
+            }
         }
         hs_bar(gr.bar_all, gr.gnt);
         if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[5] += now_ - tp; tp = now_; }
@@ -244,22 +253,27 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
             for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
         }
         const int nbmax = (bw + 7) / 8;
-        if (nbmax > 1) {
+        if (bw > SB) {
+            // snapshot of the sub-block's pivot rows; zero in the sub-block's own columns (for SB = 4 they share a DMMA
+            // column block with four columns that are updated)
             for (int e = gr.gtid; e < SB * B; e += gr.gnt) {
                 const int k = e / B, c = e % B;
-                if (c < c0 || c >= c0 + SB) Rs[k * LDR + c] = (k < ncols) ? panel[sm.prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
+                const bool own = c >= c0 && c < c0 + SB;
+                Rs[k * LDR + c] = (k < ncols && !own) ? panel[sm.prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
             }
             hs_bar(gr.bar_all, gr.gnt);
+            if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[13] += now_ - tp; tp = now_; }
             // other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs (8 x |J|) on DMMA; a warp takes 32 rows
             // and the column blocks whose running index % nbmod == nbsel
             const int rbase = gr.rbase;
             if (rbase < n) {
-                int pk[2];
+                constexpr int KQ = SB / 4;
+                int pk[KQ];
 #pragma unroll
-                for (int q = 0; q < 2; q++) pk[q] = (q * 4 + t < ncols) ? sm.prow[c0 + q * 4 + t] : -1;
-                cplx a[2][4];
+                for (int q = 0; q < KQ; q++) pk[q] = (q * 4 + t < ncols) ? sm.prow[c0 + q * 4 + t] : -1;
+                cplx a[KQ][4];
 #pragma unroll
-                for (int q = 0; q < 2; q++)
+                for (int q = 0; q < KQ; q++)
 #pragma unroll
                     for (int i = 0; i < 4; i++) {
                         const int rr = rbase + i * 8 + g;
@@ -268,7 +282,7 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
                     }
                 int cnt = 0;
                 for (int nb = 0; nb < nbmax; nb++) {
-                    if (nb == s) continue;
+                    if (SB == 8 && nb == s) continue;
                     if (((cnt++) % gr.nbmod) != gr.nbsel) continue;
                     double cre[4][2], cim[4][2];
                     cplx *Cw = panel + rbase * LDP + nb * 8;
@@ -278,7 +292,7 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
                         cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
                     }
 #pragma unroll
-                    for (int q = 0; q < 2; q++) {
+                    for (int q = 0; q < KQ; q++) {
                         const cplx bb = Rs[(q * 4 + t) * LDR + nb * 8 + g];
 #pragma unroll
                         for (int i = 0; i < 4; i++) zmma884(cre[i], cim[i], a[q][i].x, a[q][i].y, -a[q][i].y, bb.x, bb.y);
@@ -291,6 +305,7 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
                 }
             }
             hs_bar(gr.bar_all, gr.gnt);
+            if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[14] += now_ - tp; tp = now_; }
         }
     }
 }
@@ -453,40 +468,49 @@ __device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, 
     }
 }
 
-template <int RG, bool FULL>
-__device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw)
+// B fragments of a strip: its (<= 32) pivot rows, read from L2 before any row of the strip is written
+__device__ __forceinline__ void hs_strip_load_b(cplx (&bb)[8], const int *prow, const cplx *Cg, int ld, int col0, int ncols, int bw)
 {
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    cplx bb[8];
-    {
-        const bool colok = col0 + g < ncols;
+    const bool colok = col0 + g < ncols;
 #pragma unroll
-        for (int q = 0; q < 8; q++) {
-            const int k = q * 4 + t;
-            bb[q] = cmake(0.0, 0.0);
-            if (k < bw && colok) bb[q] = ldcg(Cg + (long long)prow[k] * ld + col0 + g);
-        }
+    for (int q = 0; q < 8; q++) {
+        const int k = q * 4 + t;
+        bb[q] = cmake(0.0, 0.0);
+        if (k < bw && colok) bb[q] = ldcg(Cg + (long long)prow[k] * ld + col0 + g);
     }
+}
+
+// rows [r_begin, nlim) of the strip (r_begin a multiple of 16 RG)
+template <int RG, bool FULL>
+__device__ __forceinline__ void hs_strip_rows(const cplx *panel, const cplx (&bb)[8], cplx *Cg, int ld, int r_begin, int nlim,
+                                              int col0, int ncols, int bw)
+{
+    const int lane = threadIdx.x & 31, t = lane & 3;
     const int kq = (bw + 3) >> 2;
-#ifdef HS_DIAG_NOMEM
-    const bool cok = false;
-#else
     const bool cok = col0 + 2 * t < ncols;
-#endif
     cplx *Cl = Cg + col0 + 2 * t;
     constexpr int GR = 8 * RG;
     HSAcc<RG> h0, h1;
-    hs_acc_load<RG>(h0, Cl, ld, n, 0, cok);
-    for (int r0 = 0; r0 < n; r0 += 2 * GR) {
-        hs_acc_load<RG>(h1, Cl, ld, n, r0 + GR, cok);
+    hs_acc_load<RG>(h0, Cl, ld, nlim, r_begin, cok);
+    for (int r0 = r_begin; r0 < nlim; r0 += 2 * GR) {
+        hs_acc_load<RG>(h1, Cl, ld, nlim, r0 + GR, cok);
         hs_acc_compute<RG, FULL>(h0, panel, r0, bb, kq);
-        hs_acc_store<RG>(h0, Cl, ld, n, r0, cok);
-        hs_acc_load<RG>(h0, Cl, ld, n, r0 + 2 * GR, cok);
-        if (r0 + GR < n) {
+        hs_acc_store<RG>(h0, Cl, ld, nlim, r0, cok);
+        hs_acc_load<RG>(h0, Cl, ld, nlim, r0 + 2 * GR, cok);
+        if (r0 + GR < nlim) {
             hs_acc_compute<RG, FULL>(h1, panel, r0 + GR, bb, kq);
-            hs_acc_store<RG>(h1, Cl, ld, n, r0 + GR, cok);
+            hs_acc_store<RG>(h1, Cl, ld, nlim, r0 + GR, cok);
         }
     }
+}
+
+template <int RG, bool FULL>
+__device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw)
+{
+    cplx bb[8];
+    hs_strip_load_b(bb, prow, Cg, ld, col0, ncols, bw);
+    hs_strip_rows<RG, FULL>(panel, bb, Cg, ld, 0, n, col0, ncols, bw);
 }
 
 // ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry); fills sm.perm / sm.pinv ------------------------
@@ -511,7 +535,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         cp_async_wait<0>();
         __syncthreads();
         HS_TICK(1);
-        hs_factor_panel(view, grp, n, k0, bw, used, status_slot);
+        hs_factor_panel<HS_FSB>(view, grp, n, k0, bw, used, status_slot);
         HS_TICK(2);
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
         for (int e = tid; e < n * HS_B; e += HS_NT) {
@@ -585,9 +609,11 @@ struct HSAsm {
     HSTab *tb;                         // per-row tables (alias the idle candidate buffers)
     const int *perm_prev, *pinv_prev;  // row maps of the previous half-step
 };
-template <int NT, int RB>
+// PART 0: A and W by all NT threads; 1: the tables and A only (all NT threads; ends with a barrier); 2: W only, by the
+// wnt threads wtid = 0 .. wnt-1 (no barrier; needs the tables of PART 1)
+template <int NT, int RB, int PART = 0>
 __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a, int bl, int i, int kind, bool first,
-                                            const cplx *Xp, const cplx *Wp, cplx *Xn, cplx *Wn)
+                                            const cplx *Xp, const cplx *Wp, cplx *Xn, cplx *Wn, int wtid = threadIdx.x, int wnt = NT)
 {
     constexpr int HS_NT = NT;        // threads that run the assembly (the whole CTA of either kernel)
     const int tid = threadIdx.x, M = a.M, L = a.L, ld = a.ldn, nc = M / 2;
@@ -604,6 +630,7 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
     if (first) {
         // half-step 0 (B_0): g_prev = surface Green's function of the left lead (slice -1, same atoms j), W = I
         const cplx *gl = a.gL + (long long)e * MM;
+        if (PART != 2)
         for (int idx = tid; idx < n * n; idx += HS_NT) {
             const int r = idx / n, c = idx % n, jr = 2 * r + par, jc = 2 * c + par;
             cplx v = cmake(0.0, 0.0);
@@ -611,10 +638,12 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
             if (mk[jr] && mk[jc]) { const cplx g = gl[(long long)jr * M + jc]; v.x -= t2 * g.x; v.y -= t2 * g.y; }
             Xn[(long long)r * ld + c] = v;
         }
-        for (int idx = tid; idx < n * nc; idx += HS_NT) {
+        if (PART != 1)
+        for (int idx = wtid; idx < n * nc; idx += wnt) {
             const int r = idx / nc, c = idx % nc;
             Wn[(long long)r * ld + c] = cmake(r == c ? 1.0 : 0.0, 0.0);
         }
+        if (PART == 1) __syncthreads();
         return;
     }
     const cplx *gr = a.gR + (long long)e * MM;
@@ -623,6 +652,7 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
     //   kind B: ra[r] = m'[r];                       ca[c] = m'[c] ? physical column of g_prev[.][c] : -1
     //   kind F: ra/rb[r] = lower / upper B neighbour; ca/cb[c] = physical column of that neighbour, or -1
     HSTab &tb = *sm.tb;
+    if (PART != 2) {
     if (tid < n) {
         const int r = tid;
         tb.eps[r] = E - eps[2 * r + par];
@@ -699,15 +729,17 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         }
         __syncthreads();
     }
+    }
+    if (PART == 1) return;
     // W = C P_prev: coalesced rows straight from L2, 6 independent elements per thread in flight
     const int nel = n * nc;
     constexpr int WB = 6;
-    for (int base = 0; base < nel; base += WB * HS_NT) {
+    for (int base = 0; base < nel; base += WB * wnt) {
         cplx va[WB], vb[WB];
         int rr[WB], cc[WB];
 #pragma unroll
         for (int k = 0; k < WB; k++) {
-            const int idx = base + k * HS_NT + tid;
+            const int idx = base + k * wnt + wtid;
             va[k] = cmake(0.0, 0.0); vb[k] = cmake(0.0, 0.0);
             rr[k] = -1;
             if (idx < nel) {
@@ -726,7 +758,7 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         for (int k = 0; k < WB; k++)
             if (rr[k] >= 0) Wn[(long long)rr[k] * ld + cc[k]] = cmake(a.t * (va[k].x + vb[k].x), a.t * (va[k].y + vb[k].y));
     }
-    __syncthreads();          // the tables alias the pivot-search buffers
+    if (PART == 0) __syncthreads();          // the tables alias the pivot-search buffers
 }
 
 __device__ unsigned hs_sm_arrivals[256];

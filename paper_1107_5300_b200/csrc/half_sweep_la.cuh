@@ -15,7 +15,14 @@
 
 namespace rgf {
 
-constexpr int LA_NT = 512, LA_NF = 128;          // threads per CTA, threads of the factor group
+#ifndef LA_FSMSP
+#define LA_FSMSP 1
+#endif
+#ifndef LA_NT_
+#define LA_NT_ 512
+#endif
+constexpr int LA_NT = LA_NT_, LA_NF = 128;       // threads per CTA, threads of the factor group
+constexpr int LA_U0 = LA_FSMSP ? 32 : LA_NF;        // first update thread (profiling)
 constexpr int LA_RB = 32;                        // output rows per staging block of the assembly
 
 struct HSmemLA {
@@ -26,14 +33,16 @@ struct HSmemLA {
     alignas(16) unsigned ckey[2 * (HS_NT / 32)];
     int perm[HS_NMAX], pinv[HS_NMAX], perm_prev[HS_NMAX], pinv_prev[HS_NMAX];
     int prow[2][HS_B];
+    int next;                                    // next strip of the current update (dynamic distribution over the warps)
+    HSTab tab;                                   // tables of the assembly (W is assembled while panel 0 is factored)
     long long prof[16];
 };
 static_assert(2 * (LA_RB + 2) * HS_NMAX <= 2 * HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffers");
 
 // panel columns [k0, k0 + bw) of X -> shared memory, by the factor group (cp.async.cg: L2, never a stale L1 line)
-__device__ __forceinline__ void la_load_panel(cplx *panel, const cplx *X, int ld, int n, int k0, int bw)
+__device__ __forceinline__ void la_load_panel(cplx *panel, const cplx *X, int ld, int n, int k0, int bw, int ftid)
 {
-    for (int e = threadIdx.x; e < HS_NMAX * HS_B; e += LA_NF) {
+    for (int e = ftid; e < HS_NMAX * HS_B; e += LA_NF) {
         const int rr = e / HS_B, c = e % HS_B;
         const bool ok = rr < n && c < bw;
         cp_async16(panel + rr * HS_LDP + c, ok ? X + (long long)rr * ld + k0 + c : X, ok ? 16 : 0);
@@ -50,28 +59,45 @@ __device__ __forceinline__ void la_strip(const cplx *panel, const int *prow, cpl
 }
 
 // ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry); fills sm.perm / sm.pinv ------------------------
-__device__ __forceinline__ void la_gauss_jordan(HSmemLA &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof)
+// wfn() is run by the update warps while the factor warps factor the first panel (the assembly of W, which no one
+// needs before the first update).
+template <class WFn>
+__device__ __forceinline__ void la_gauss_jordan(HSmemLA &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof, WFn &&wfn)
 {
     long long tc = prof ? clock64() : 0;
 #define LA_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
     const int tid = threadIdx.x, warp = tid >> 5;
+#if LA_FSMSP
+    // factor warps = warps 0, 4, 8, 12: all on SM sub-partition 0 (warp id mod 4), which then runs no update warp while
+    // a panel is factored.  A DFMA that competes with two or more warps streaming DMMAs on its sub-partition is starved
+    // (measured: 8 -> 82 cycles per dependent DFMA beside one such warp, > 30 000 beside two), so the pivot chain must
+    // not share a sub-partition with the updates.
+    const bool isF = (warp & 3) == 0;
+    const int fslot = warp >> 2, ftid = (fslot << 5) | (tid & 31);
+    const int utid = ((warp >> 2) * 3 + (warp & 3) - 1) * 32 + (tid & 31);       // index among the update threads
+#else
     const bool isF = warp < LA_NF / 32;
-    bool used = !(tid < n);
+    const int fslot = warp, ftid = tid;
+    const int utid = tid - LA_NF;
+#endif
+    bool used = !(ftid < n);
     HSGroup grp;
-    grp.r = tid; grp.slot = warp; grp.nslots = (n + 31) >> 5; grp.gtid = tid; grp.gnt = LA_NF;
+    grp.r = ftid; grp.slot = fslot; grp.nslots = (n + 31) >> 5; grp.gtid = ftid; grp.gnt = LA_NF;
     grp.bar_pivot = 1; grp.n_pivot = grp.nslots * 32; grp.bar_all = 2;
-    grp.rbase = warp * 32; grp.nbsel = 0; grp.nbmod = 1;
+    grp.rbase = fslot * 32; grp.nbsel = 0; grp.nbmod = 1;
     HSView view;
     view.Rs = sm.Rs; view.crow = sm.crow; view.cinv = sm.cinv; view.ckey = sm.ckey;
-    view.perm = sm.perm; view.pinv = sm.pinv; view.prof = nullptr;
+    view.perm = sm.perm; view.pinv = sm.pinv; view.prof = prof ? sm.prof : nullptr;
     const int np = (n + HS_B - 1) / HS_B;
     const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3;
-    // first panel: nothing to overlap it with
+    // first panel: only the assembly of W runs beside it
     if (isF) {
         const int bw0 = n < HS_B ? n : HS_B;
-        la_load_panel(sm.panel[0], X, ld, n, 0, bw0);
+        la_load_panel(sm.panel[0], X, ld, n, 0, bw0, ftid);
         view.panel = sm.panel[0]; view.prow = sm.prow[0];
-        hs_factor_panel(view, grp, n, 0, bw0, used, status_slot);
+        hs_factor_panel<HS_FSB>(view, grp, n, 0, bw0, used, status_slot);
+    } else {
+        wfn(utid);
     }
     __syncthreads();
     LA_TICK(2);
@@ -79,37 +105,61 @@ __device__ __forceinline__ void la_gauss_jordan(HSmemLA &sm, cplx *X, cplx *W, i
         const int cur = p & 1, k0 = p * HS_B, bw = (n - k0 < HS_B) ? (n - k0) : HS_B;
         cplx *panel = sm.panel[cur];
         const int *prow = sm.prow[cur];
+        const bool more = p + 1 < np;
+        const int sk0 = k0 >> 3;
+        const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;                    // strips of panel p: [sk0, sk1)
+        const int sn1 = more ? ((sk1 + HS_B / 8 < nsx) ? sk1 + HS_B / 8 : nsx) : sk1;     // strips of panel p+1: [sk1, sn1)
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
         for (int e = tid; e < n * HS_B; e += LA_NT) {
             const int rr = e / HS_B, c = e % HS_B;
             if (c < bw) X[(long long)rr * ld + k0 + c] = panel[rr * HS_LDP + c];
         }
         __syncthreads();
-        if (tid < bw) panel[prow[tid] * HS_LDP + tid].x -= 1.0;
-        __syncthreads();
-        LA_TICK(3);
-        const bool more = p + 1 < np;
-        const int sk0 = k0 >> 3;
-        const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;                    // strips of panel p: [sk0, sk1)
-        const int sn1 = more ? ((sk1 + HS_B / 8 < nsx) ? sk1 + HS_B / 8 : nsx) : sk1;     // strips of panel p+1: [sk1, sn1)
-        if (more && isF) {
-            const int s = sk1 + warp;
-            if (s < sn1) la_strip(panel, prow, X, ld, n, s * 8, n, bw);
-            hs_bar(2, LA_NF);
-            const int k1 = k0 + HS_B, bw1 = (n - k1 < HS_B) ? (n - k1) : HS_B;
-            la_load_panel(sm.panel[cur ^ 1], X, ld, n, k1, bw1);
-            view.panel = sm.panel[cur ^ 1]; view.prow = sm.prow[cur ^ 1];
-            hs_factor_panel(view, grp, n, k1, bw1, used, status_slot);
-        } else {
-            // every other strip of X, then the strips of W, over the update warps (all warps behind the last panel)
-            const int nw = more ? (LA_NT - LA_NF) / 32 : LA_NT / 32, w0 = more ? warp - LA_NF / 32 : warp;
-            const int nxs = nsx - (sn1 - sk0), tot = nxs + nsw;
-            for (int s = w0; s < tot; s += nw) {
-                if (s < nxs) la_strip(panel, prow, X, ld, n, (s < sk0 ? s : s + (sn1 - sk0)) * 8, n, bw);
-                else la_strip(panel, prow, W, ld, n, (s - nxs) * 8, nc, bw);
+        if (tid < bw) panel[prow[tid] * HS_LDP + tid].x -= 1.0;      // (any bw threads)
+        if (tid == 0) sm.next = 0;
+        long long tq = prof ? clock64() : 0;
+#define LA_TOCK(slot, who) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == (who)) { sm.prof[slot] += now_ - tq; tq = now_; } } } while (0)
+        if (more) {
+            // the strips that hold panel p+1 come first, split over all 16 warps (strip = warp & 3, 32 rows each): every
+            // warp reads its strip's pivot rows before the barrier, writes after it
+            constexpr int PARTS = LA_NT / 128, RPP = ((HS_NMAX / PARTS + 15) / 16) * 16;
+            const int s = sk1 + (warp & 3), r_begin = (warp >> 2) * RPP, nlim = (r_begin + RPP < n) ? r_begin + RPP : n;
+            const bool act = s < sn1 && r_begin < n;
+            cplx bb[8];
+            if (act) hs_strip_load_b(bb, prow, X, ld, s * 8, n, bw);
+            __syncthreads();
+            if (act) {
+                if (bw == HS_B) hs_strip_rows<HS_RG, true>(panel, bb, X, ld, r_begin, nlim, s * 8, n, bw);
+                else hs_strip_rows<HS_RG, false>(panel, bb, X, ld, r_begin, nlim, s * 8, n, bw);
             }
         }
         __syncthreads();
+        LA_TICK(3);
+        LA_TOCK(12, 0);
+        if (more && isF) {
+            const int k1 = k0 + HS_B, bw1 = (n - k1 < HS_B) ? (n - k1) : HS_B;
+            la_load_panel(sm.panel[cur ^ 1], X, ld, n, k1, bw1, ftid);
+            LA_TOCK(6, 0);
+            view.panel = sm.panel[cur ^ 1]; view.prow = sm.prow[cur ^ 1];
+            hs_factor_panel<HS_FSB>(view, grp, n, k1, bw1, used, status_slot);
+            LA_TOCK(7, 0);
+        }
+        {
+            // every other strip of X and the strips of W, handed out dynamically: the update warps start at once, the
+            // factor warps join when panel p+1 is factored
+            const int nxs = nsx - (sn1 - sk0), tot = nxs + nsw;
+            for (;;) {
+                int s = 0;
+                if ((tid & 31) == 0) s = atomicAdd(&sm.next, 1);
+                s = __shfl_sync(0xffffffffu, s, 0);
+                if (s >= tot) break;
+                if (s < nsw) la_strip(panel, prow, W, ld, n, s * 8, nc, bw);
+                else { const int sx = s - nsw; la_strip(panel, prow, X, ld, n, (sx < sk0 ? sx : sx + (sn1 - sk0)) * 8, n, bw); }
+            }
+            if (more) LA_TOCK(8, LA_U0); else { LA_TOCK(9, LA_U0); }
+        }
+        __syncthreads();
+        if (more) { LA_TOCK(10, LA_U0); LA_TOCK(11, 0); }
         LA_TICK(4);
     }
 #undef LA_TICK
@@ -139,7 +189,7 @@ __global__ void __launch_bounds__(LA_NT, 1) half_sweep_la_kernel(HSweepArgs a)
         __syncthreads();
     }
     if (tid < 16) sm.prof[tid] = 0;
-    const HSAsm av = {&sm.panel[0][0], reinterpret_cast<HSTab *>(sm.crow), sm.perm_prev, sm.pinv_prev};
+    const HSAsm av = {&sm.panel[0][0], &sm.tab, sm.perm_prev, sm.pinv_prev};
     int n = 0;
     for (int hs = hs_begin; hs < hs_end; hs++) {
         const int i = hs >> 1, kind = hs & 1;
@@ -147,11 +197,12 @@ __global__ void __launch_bounds__(LA_NT, 1) half_sweep_la_kernel(HSweepArgs a)
         if (tid < HS_NMAX) { sm.perm_prev[tid] = sm.perm[tid]; sm.pinv_prev[tid] = sm.pinv[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
-        hs_assemble<LA_NT, LA_RB>(av, a, bl, i, kind, hs == 0, Xp, Wp, Xn, Wn);
-        __syncthreads();
+        hs_assemble<LA_NT, LA_RB, 1>(av, a, bl, i, kind, hs == 0, Xp, Wp, Xn, Wn);
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         n = half_count(M, kind == 0 ? ((i + 1) & 1) : (i & 1));
-        la_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr);
+        la_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr, [&](int utid) {
+            hs_assemble<LA_NT, LA_RB, 2>(av, a, bl, i, kind, hs == 0, Xp, Wp, Xn, Wn, utid, LA_NT - LA_NF);
+        });
     }
     if (tid < HS_NMAX) gperm[tid] = sm.perm[tid];
     if (a.prof && tid < 16) a.prof[bl * 16 + tid] += sm.prof[tid];

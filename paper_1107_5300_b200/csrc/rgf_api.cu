@@ -598,8 +598,8 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
         double s[16] = {0};
         for (int b = 0; b < nb; b++) for (int k = 0; k < 16; k++) s[k] += (double)h[16 * (size_t)b + k];
         const double hsn = (double)nb * a.hs_end;
-        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           update loop: load1 %.0f sync %.0f stageR %.0f comp0 %.0f store0 %.0f load0 %.0f comp1 %.0f store1 %.0f\n",
-                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[8] / hsn, s[9] / hsn, s[10] / hsn, s[11] / hsn, s[12] / hsn, s[13] / hsn, s[14] / hsn, s[15] / hsn);
+        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           slots 8-15: %.0f %.0f %.0f %.0f %.0f %.0f %.0f %.0f   slots 5-7: %.0f %.0f %.0f\n",
+                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[8] / hsn, s[9] / hsn, s[10] / hsn, s[11] / hsn, s[12] / hsn, s[13] / hsn, s[14] / hsn, s[15] / hsn, s[5] / hsn, s[6] / hsn, s[7] / hsn);
     }
     return RGF_OK;
 }
