@@ -47,19 +47,22 @@ struct HSweepArgs {
     int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
                                   // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
     long long *prof;              // optional [nb][16] cycle counters of thread 0 per phase (NULL = off)
-    int stagger;                  // cycles the second CTA to arrive on an SM waits before its first half-step (see the kernel)
     cplx *g_out, *P_out;          // after half-step hs_end - 1: g dense n x n (ld n) and P (ld nh), stride nh*nh; may be NULL
 };
 
 struct HSmem {
     cplx panel[HS_NMAX * HS_LDP];
-    cplx R[2][HS_B * HS_LDR];
+    cplx Rs[HS_SB * HS_LDR];     // pivot rows of a sub-block (in-panel update)
     cplx crow[2 * (HS_NT / 32) * HS_SB];
     cplx cinv[2 * (HS_NT / 32)];
     alignas(16) unsigned ckey[2 * (HS_NT / 32)];
-    int perm[HS_NMAX], pinv[HS_NMAX], perm_prev[HS_NMAX], pinv_prev[HS_NMAX];
+    int perm[HS_NMAX], pinv[HS_NMAX];                 // of the running elimination: pivot row of a column and its inverse
+    int rmap[HS_NMAX], cmap[HS_NMAX];                 // logical row / column of the last result -> physical row / column
+    int rmap_prev[HS_NMAX], cmap_prev[HS_NMAX];
     int prow[HS_B];
-    int flag;
+    // in-place assembly of a kind-B half-step (HSXf), per physical row / column of the previous result
+    double xf_sr[HS_NMAX], xf_sw[HS_NMAX], xf_dre[HS_NMAX], xf_mc[HS_NMAX];
+    short xf_dcol[HS_NMAX];
     long long prof[16];          // per-phase cycle counters of thread 0 (debugging aid, RGF_HS_PROF)
 };
 
@@ -204,6 +207,60 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
 #undef HS_DBGT
 }
 
+// in-panel update behind sub-block s (columns [c0, c0 + ncols) of the panel, pivot rows snapshotted in sm.Rs):
+// panel[:, J] += (N'_s - E_s) (n x SB) * Rs (SB x |J|) on DMMA; a warp takes the 32 rows from gr.rbase and the column blocks
+// whose running index % gr.nbmod == gr.nbsel
+template <int SB>
+__device__ __forceinline__ void hs_inpanel_update(const HSView &sm, const HSGroup &gr, int n, int bw, int s, int c0, int ncols)
+{
+    constexpr int LDP = HS_LDP, LDR = HS_LDR;
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    cplx *panel = sm.panel;
+    const cplx *Rs = sm.Rs;
+    const int nbmax = (bw + 7) / 8;
+    // other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs (8 x |J|) on DMMA; a warp takes 32 rows
+    // and the column blocks whose running index % nbmod == nbsel
+    const int rbase = gr.rbase;
+    if (rbase < n) {
+        constexpr int KQ = SB / 4;
+        int pk[KQ];
+#pragma unroll
+        for (int q = 0; q < KQ; q++) pk[q] = (q * 4 + t < ncols) ? sm.prow[c0 + q * 4 + t] : -1;
+        cplx a[KQ][4];
+#pragma unroll
+        for (int q = 0; q < KQ; q++)
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                const int rr = rbase + i * 8 + g;
+                a[q][i] = panel[rr * LDP + c0 + q * 4 + t];
+                if (rr == pk[q]) a[q][i].x -= 1.0;
+            }
+        int cnt = 0;
+        for (int nb = 0; nb < nbmax; nb++) {
+            if (SB == 8 && nb == s) continue;
+            if (((cnt++) % gr.nbmod) != gr.nbsel) continue;
+            double cre[4][2], cim[4][2];
+            cplx *Cw = panel + rbase * LDP + nb * 8;
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                const cplx v0 = Cw[(i * 8 + g) * LDP + 2 * t], v1 = Cw[(i * 8 + g) * LDP + 2 * t + 1];
+                cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
+            }
+#pragma unroll
+            for (int q = 0; q < KQ; q++) {
+                const cplx bb = Rs[(q * 4 + t) * LDR + nb * 8 + g];
+#pragma unroll
+                for (int i = 0; i < 4; i++) zmma884(cre[i], cim[i], a[q][i].x, a[q][i].y, -a[q][i].y, bb.x, bb.y);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                Cw[(i * 8 + g) * LDP + 2 * t] = cmake(cre[i][0], cim[i][0]);
+                Cw[(i * 8 + g) * LDP + 2 * t + 1] = cmake(cre[i][1], cim[i][1]);
+            }
+        }
+    }
+}
+
 // ---- panel factorisation in shared memory: columns [k0, k0 + bw) of all n rows --------------------
 // On entry sm.panel[r][c] = X[r][k0 + c] (zero for c >= bw, r >= n).  On exit sm.panel = N' (the
 // transformed columns), sm.prow[c] = pivot row of column k0 + c, perm / pinv updated, used |= pivot.
@@ -214,7 +271,6 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
 {
     constexpr int B = HS_B, LDP = HS_LDP, LDR = HS_LDR;
     static_assert(SB == 8 || SB == 4, "sub-block width");
-    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int r = gr.r;
     const bool has_row = r < n;
     long long tp = sm.prof ? clock64() : 0;
@@ -252,7 +308,6 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
 #pragma unroll
             for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
         }
-        const int nbmax = (bw + 7) / 8;
         if (bw > SB) {
             // snapshot of the sub-block's pivot rows; zero in the sub-block's own columns (for SB = 4 they share a DMMA
             // column block with four columns that are updated)
@@ -263,47 +318,7 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
             }
             hs_bar(gr.bar_all, gr.gnt);
             if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[13] += now_ - tp; tp = now_; }
-            // other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs (8 x |J|) on DMMA; a warp takes 32 rows
-            // and the column blocks whose running index % nbmod == nbsel
-            const int rbase = gr.rbase;
-            if (rbase < n) {
-                constexpr int KQ = SB / 4;
-                int pk[KQ];
-#pragma unroll
-                for (int q = 0; q < KQ; q++) pk[q] = (q * 4 + t < ncols) ? sm.prow[c0 + q * 4 + t] : -1;
-                cplx a[KQ][4];
-#pragma unroll
-                for (int q = 0; q < KQ; q++)
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        const int rr = rbase + i * 8 + g;
-                        a[q][i] = panel[rr * LDP + c0 + q * 4 + t];
-                        if (rr == pk[q]) a[q][i].x -= 1.0;
-                    }
-                int cnt = 0;
-                for (int nb = 0; nb < nbmax; nb++) {
-                    if (SB == 8 && nb == s) continue;
-                    if (((cnt++) % gr.nbmod) != gr.nbsel) continue;
-                    double cre[4][2], cim[4][2];
-                    cplx *Cw = panel + rbase * LDP + nb * 8;
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        const cplx v0 = Cw[(i * 8 + g) * LDP + 2 * t], v1 = Cw[(i * 8 + g) * LDP + 2 * t + 1];
-                        cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
-                    }
-#pragma unroll
-                    for (int q = 0; q < KQ; q++) {
-                        const cplx bb = Rs[(q * 4 + t) * LDR + nb * 8 + g];
-#pragma unroll
-                        for (int i = 0; i < 4; i++) zmma884(cre[i], cim[i], a[q][i].x, a[q][i].y, -a[q][i].y, bb.x, bb.y);
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        Cw[(i * 8 + g) * LDP + 2 * t] = cmake(cre[i][0], cim[i][0]);
-                        Cw[(i * 8 + g) * LDP + 2 * t + 1] = cmake(cre[i][1], cim[i][1]);
-                    }
-                }
-            }
+            hs_inpanel_update<SB>(sm, gr, n, bw, s, c0, ncols);
             hs_bar(gr.bar_all, gr.gnt);
             if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[14] += now_ - tp; tp = now_; }
         }
@@ -314,7 +329,7 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
 __device__ __forceinline__ HSView hs_view(HSmem &sm, bool prof)
 {
     HSView v;
-    v.panel = sm.panel; v.Rs = sm.R[0]; v.crow = sm.crow; v.cinv = sm.cinv; v.ckey = sm.ckey;
+    v.panel = sm.panel; v.Rs = sm.Rs; v.crow = sm.crow; v.cinv = sm.cinv; v.ckey = sm.ckey;
     v.prow = sm.prow; v.perm = sm.perm; v.pinv = sm.pinv; v.prof = prof ? sm.prof : nullptr;
     return v;
 }
@@ -328,76 +343,31 @@ __device__ __forceinline__ HSGroup hs_group_cta(int n)
     return g;
 }
 
-// ---- R = C[prow[0..bw)][col0 .. col0+32) -> shared memory (cp.async.cg: L2, never a stale L1 line) --------
-__device__ __forceinline__ void hs_stage_R(HSmem &sm, int buf, const cplx *Cg, int ld, int col0, int ncols, int bw)
+// ---- in-place assembly of a kind-B half-step, applied to an element while it is loaded ---------------------------
+// A_B = z - eps_B - t^2 m' (.) gF_prev (.) m' and W_B = t m' (.) PF_prev are the previous result scaled element by
+// element plus a diagonal (half_kernels.cuh): nothing moves, so the previous result is left where it is (rows and
+// columns in the permuted order the elimination produced) and turned into [A | W] on the fly by whoever loads an
+// element first -- the load of panel 0 and the strips of its update touch every element exactly once.  Tables are per
+// PHYSICAL row rho / column gamma of the previous result:  x' = sr[rho] mc[gamma] x  (+ (dre[rho], eta) at gamma =
+// dcol[rho], the position of the atom's own diagonal element),  w' = sw[rho] w.
+struct HSXf {
+    const double *sr, *sw, *dre, *mc;
+    const short *dcol;
+    double eta;
+};
+// TF: 0 = plain load, 1 = element of X, 2 = element of W
+template <int TF>
+__device__ __forceinline__ cplx hs_xf(const HSXf &xf, cplx v, int rho, int gamma)
 {
-    cplx *R = sm.R[buf];
-#pragma unroll
-    for (int it = 0; it < (HS_B * HS_B) / HS_NT; it++) {
-        const int e = threadIdx.x + it * HS_NT, k = e / HS_B, c = e % HS_B;
-        const bool ok = k < bw && col0 + c < ncols;
-        cp_async16(R + k * HS_LDR + c, ok ? Cg + (long long)sm.prow[k] * ld + col0 + c : Cg, ok ? 16 : 0);
+    if (TF == 1) {
+        const double sc = xf.sr[rho] * xf.mc[gamma];
+        v.x *= sc; v.y *= sc;
+        if (gamma == xf.dcol[rho]) { v.x += xf.dre[rho]; v.y += xf.eta; }
+    } else if (TF == 2) {
+        const double sc = xf.sw[rho];
+        v.x *= sc; v.y *= sc;
     }
-    cp_async_commit();
-}
-
-// ---- C[:, col0 .. col0+16) += Mult (n x 32, sm.panel) * R[:, rc0 .. rc0+16) (sm.R[buf]), in place in L2 -----------
-// warp w owns rows [16 w, 16 w + 16); a half-tile is 2 x 2 DMMA blocks of 8 x 8 complex (16 accumulator doubles).
-// Load / compute / store are separate so that the caller can keep the next half-tile's loads in flight while
-// this one is on the tensor pipe (the register budget of 128 has no room for a second full 16 x 32 tile).
-struct HSHalf { double re[2][2][2], im[2][2][2]; };
-
-__device__ __forceinline__ void hs_half_load(HSHalf &h, const cplx *Cg, int ld, int n, int col0, int ncols)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
-#pragma unroll
-    for (int i = 0; i < 2; i++) {
-        const int rr = warp * 16 + i * 8 + g;
-        const cplx *src = Cg + (long long)rr * ld + col0 + 2 * t;
-#pragma unroll
-        for (int j = 0; j < 2; j++) {
-            // elements (rr, c) and (rr, c + 1), c even: one 32-byte sector, one LDG.256 (two 16-byte loads would each
-            // touch half a sector and double the L2 transactions).  c + 1 may be the padding column (ld is even).
-            double r0 = 0.0, i0 = 0.0, r1 = 0.0, i1 = 0.0;
-            if (rr < n && col0 + j * 8 + 2 * t < ncols) ld256cg(src + j * 8, r0, i0, r1, i1);
-            h.re[i][j][0] = r0; h.im[i][j][0] = i0; h.re[i][j][1] = r1; h.im[i][j][1] = i1;
-        }
-    }
-}
-
-__device__ __forceinline__ void hs_half_compute(HSHalf &h, const HSmem &sm, int buf, int rc0, int kmax)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
-    const cplx *cA = sm.panel + warp * 16 * HS_LDP;
-    const cplx *cB = sm.R[buf] + rc0;
-    // kmax = panel width rounded up to 4 (Mult columns / R rows beyond the panel width are zero)
-#pragma unroll 2
-    for (int kk = 0; kk < kmax; kk += 4) {
-        cplx a[2], bb[2];
-#pragma unroll
-        for (int i = 0; i < 2; i++) a[i] = cA[(i * 8 + g) * HS_LDP + kk + t];
-#pragma unroll
-        for (int j = 0; j < 2; j++) bb[j] = cB[(kk + t) * HS_LDR + j * 8 + g];
-#pragma unroll
-        for (int i = 0; i < 2; i++) {
-            const double nai = -a[i].y;
-#pragma unroll
-            for (int j = 0; j < 2; j++) zmma884(h.re[i][j], h.im[i][j], a[i].x, a[i].y, nai, bb[j].x, bb[j].y);
-        }
-    }
-}
-
-__device__ __forceinline__ void hs_half_store(const HSHalf &h, cplx *Cg, int ld, int n, int col0, int ncols)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
-#pragma unroll
-    for (int i = 0; i < 2; i++) {
-        const int rr = warp * 16 + i * 8 + g;
-        cplx *dst = Cg + (long long)rr * ld + col0 + 2 * t;
-#pragma unroll
-        for (int j = 0; j < 2; j++)
-            if (rr < n && col0 + j * 8 + 2 * t < ncols) st256(dst + j * 8, h.re[i][j][0], h.im[i][j][0], h.re[i][j][1], h.im[i][j][1]);
-    }
+    return v;
 }
 
 // ---- barrier-free update of one 8-column strip: C[:, col0 .. col0+8) += Mult (n x 32, sm.panel) * R ---------------
@@ -408,26 +378,33 @@ __device__ __forceinline__ void hs_half_store(const HSHalf &h, cplx *Cg, int ld,
 template <int RG>
 struct HSAcc { double re[RG][2], im[RG][2]; };
 
-template <int RG>
-__device__ __forceinline__ void hs_acc_load(HSAcc<RG> &h, const cplx *Cg, int ld, int n, int r0, bool cok)
+template <int RG, int TF>
+__device__ __forceinline__ void hs_acc_load(HSAcc<RG> &h, const cplx *Cl, int ld, int n, int r0, bool cok, const HSXf &xf, int gamma0)
 {
     const int lane = threadIdx.x & 31, g = lane >> 2;
 #pragma unroll
     for (int i = 0; i < RG; i++) {
         const int rr = r0 + i * 8 + g;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        if (rr < n && cok) ld256cg(Cg + (long long)rr * ld, a0, a1, a2, a3);
+        if (rr < n && cok) {
+            // elements (rr, c) and (rr, c + 1), c even: one 32-byte sector, one LDG.256.  c + 1 may be the padding column.
+            ld256cg(Cl + (long long)rr * ld, a0, a1, a2, a3);
+            if (TF) {
+                const cplx v0 = hs_xf<TF>(xf, cmake(a0, a1), rr, gamma0), v1 = hs_xf<TF>(xf, cmake(a2, a3), rr, gamma0 + 1);
+                a0 = v0.x; a1 = v0.y; a2 = v1.x; a3 = v1.y;
+            }
+        }
         h.re[i][0] = a0; h.im[i][0] = a1; h.re[i][1] = a2; h.im[i][1] = a3;
     }
 }
 template <int RG>
-__device__ __forceinline__ void hs_acc_store(const HSAcc<RG> &h, cplx *Cg, int ld, int n, int r0, bool cok)
+__device__ __forceinline__ void hs_acc_store(const HSAcc<RG> &h, cplx *Cl, int ld, int n, int r0, bool cok)
 {
     const int lane = threadIdx.x & 31, g = lane >> 2;
 #pragma unroll
     for (int i = 0; i < RG; i++) {
         const int rr = r0 + i * 8 + g;
-        if (rr < n && cok) st256(Cg + (long long)rr * ld, h.re[i][0], h.im[i][0], h.re[i][1], h.im[i][1]);
+        if (rr < n && cok) st256(Cl + (long long)rr * ld, h.re[i][0], h.im[i][0], h.re[i][1], h.im[i][1]);
     }
 }
 template <int RG, bool FULL>
@@ -446,13 +423,8 @@ __device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, 
 #pragma unroll
                 for (int i = 0; i < RG; i++) a[(q + 1) & 1][i] = cA[i * 8 * HS_LDP + (q + 1) * 4];
             }
-#ifndef HS_DIAG_NOMMA
 #pragma unroll
             for (int i = 0; i < RG; i++) zmma884(h.re[i], h.im[i], a[q & 1][i].x, a[q & 1][i].y, -a[q & 1][i].y, bb[q].x, bb[q].y);
-#else
-#pragma unroll
-            for (int i = 0; i < RG; i++) { h.re[i][0] += a[q & 1][i].x * bb[q].x; h.im[i][1] += a[q & 1][i].y * bb[q].y; }
-#endif
         }
     } else {
 #pragma unroll
@@ -468,54 +440,49 @@ __device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, 
     }
 }
 
-// B fragments of a strip: its (<= 32) pivot rows, read from L2 before any row of the strip is written
-__device__ __forceinline__ void hs_strip_load_b(cplx (&bb)[8], const int *prow, const cplx *Cg, int ld, int col0, int ncols, int bw)
+// Mult columns / R rows beyond the panel width are zero, so a narrow last panel only skips DMMAs (FULL = false).
+template <int RG, bool FULL, int TF>
+__device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw,
+                                                const HSXf &xf)
 {
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    const bool colok = col0 + g < ncols;
+    // B fragments: the strip's (<= 32) pivot rows, read from L2 before any row of the strip is written
+    cplx bb[8];
+    {
+        const bool colok = col0 + g < ncols;
 #pragma unroll
-    for (int q = 0; q < 8; q++) {
-        const int k = q * 4 + t;
-        bb[q] = cmake(0.0, 0.0);
-        if (k < bw && colok) bb[q] = ldcg(Cg + (long long)prow[k] * ld + col0 + g);
+        for (int q = 0; q < 8; q++) {
+            const int k = q * 4 + t;
+            bb[q] = cmake(0.0, 0.0);
+            if (k < bw && colok) {
+                const int rho = prow[k];
+                bb[q] = hs_xf<TF>(xf, ldcg(Cg + (long long)rho * ld + col0 + g), rho, col0 + g);
+            }
+        }
     }
-}
-
-// rows [r_begin, nlim) of the strip (r_begin a multiple of 16 RG)
-template <int RG, bool FULL>
-__device__ __forceinline__ void hs_strip_rows(const cplx *panel, const cplx (&bb)[8], cplx *Cg, int ld, int r_begin, int nlim,
-                                              int col0, int ncols, int bw)
-{
-    const int lane = threadIdx.x & 31, t = lane & 3;
     const int kq = (bw + 3) >> 2;
-    const bool cok = col0 + 2 * t < ncols;
-    cplx *Cl = Cg + col0 + 2 * t;
+    const int gamma0 = col0 + 2 * t;
+    const bool cok = gamma0 < ncols;
+    cplx *Cl = Cg + gamma0;
     constexpr int GR = 8 * RG;
     HSAcc<RG> h0, h1;
-    hs_acc_load<RG>(h0, Cl, ld, nlim, r_begin, cok);
-    for (int r0 = r_begin; r0 < nlim; r0 += 2 * GR) {
-        hs_acc_load<RG>(h1, Cl, ld, nlim, r0 + GR, cok);
+    hs_acc_load<RG, TF>(h0, Cl, ld, n, 0, cok, xf, gamma0);
+    for (int r0 = 0; r0 < n; r0 += 2 * GR) {
+        hs_acc_load<RG, TF>(h1, Cl, ld, n, r0 + GR, cok, xf, gamma0);
         hs_acc_compute<RG, FULL>(h0, panel, r0, bb, kq);
-        hs_acc_store<RG>(h0, Cl, ld, nlim, r0, cok);
-        hs_acc_load<RG>(h0, Cl, ld, nlim, r0 + 2 * GR, cok);
-        if (r0 + GR < nlim) {
+        hs_acc_store<RG>(h0, Cl, ld, n, r0, cok);
+        hs_acc_load<RG, TF>(h0, Cl, ld, n, r0 + 2 * GR, cok, xf, gamma0);
+        if (r0 + GR < n) {
             hs_acc_compute<RG, FULL>(h1, panel, r0 + GR, bb, kq);
-            hs_acc_store<RG>(h1, Cl, ld, nlim, r0 + GR, cok);
+            hs_acc_store<RG>(h1, Cl, ld, n, r0 + GR, cok);
         }
     }
 }
 
-template <int RG, bool FULL>
-__device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw)
-{
-    cplx bb[8];
-    hs_strip_load_b(bb, prow, Cg, ld, col0, ncols, bw);
-    hs_strip_rows<RG, FULL>(panel, bb, Cg, ld, 0, n, col0, ncols, bw);
-}
-
-// ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry); fills sm.perm / sm.pinv ------------------------
-template <int MODE>
-__device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof)
+// ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry, or, with inplace, the previous result that HSXf turns
+// into [A | W] while panel 0 is loaded and applied); fills sm.perm / sm.pinv ---------------------------------------
+__device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof,
+                                                bool inplace, const HSXf &xf)
 {
     long long tc = prof ? clock64() : 0;
 #define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
@@ -523,16 +490,37 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
     bool used = !(tid < n);
     const HSView view = hs_view(sm, prof != nullptr);
     const HSGroup grp = hs_group_cta(n);
-    const int nchm = (n + HS_B - 1) / HS_B, ncha = (nc + HS_B - 1) / HS_B;
+    const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3;
     for (int k0 = 0; k0 < n; k0 += HS_B) {
         const int bw = (n - k0 < HS_B) ? (n - k0) : HS_B;
-        for (int e = tid; e < HS_NMAX * HS_B; e += HS_NT) {
-            const int rr = e / HS_B, c = e % HS_B;
-            const bool ok = rr < n && c < bw;
-            cp_async16(sm.panel + rr * HS_LDP + c, ok ? X + (long long)rr * ld + k0 + c : X, ok ? 16 : 0);
+        const bool tf = inplace && k0 == 0;
+        if (!tf) {
+            for (int e = tid; e < HS_NMAX * HS_B; e += HS_NT) {
+                const int rr = e / HS_B, c = e % HS_B;
+                const bool ok = rr < n && c < bw;
+                cp_async16(sm.panel + rr * HS_LDP + c, ok ? X + (long long)rr * ld + k0 + c : X, ok ? 16 : 0);
+            }
+            cp_async_commit();
+            cp_async_wait<0>();
+        } else {
+            // panel 0 of an in-place half-step: transformed on its way to shared memory, 8 loads in flight per thread
+            constexpr int PER = 8;
+            for (int e0 = 0; e0 < HS_NMAX * HS_B; e0 += PER * HS_NT) {
+                cplx v[PER];
+#pragma unroll
+                for (int k = 0; k < PER; k++) {
+                    const int e = e0 + k * HS_NT + tid, rr = e / HS_B, c = e % HS_B;
+                    v[k] = cmake(0.0, 0.0);
+                    if (rr < n && c < bw) v[k] = ldcg(X + (long long)rr * ld + c);
+                }
+#pragma unroll
+                for (int k = 0; k < PER; k++) {
+                    const int e = e0 + k * HS_NT + tid, rr = e / HS_B, c = e % HS_B;
+                    if (rr < n && c < bw) v[k] = hs_xf<1>(xf, v[k], rr, c);
+                    sm.panel[rr * HS_LDP + c] = v[k];
+                }
+            }
         }
-        cp_async_commit();
-        cp_async_wait<0>();
         __syncthreads();
         HS_TICK(1);
         hs_factor_panel<HS_FSB>(view, grp, n, k0, bw, used, status_slot);
@@ -544,56 +532,23 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         }
         __syncthreads();
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
-        if constexpr (MODE == 1) {
-            // strip list: the 8-column strips of X except the panel's own four, then the strips of W; warp w takes
-            // strips w, w + 8, ...
-            __syncthreads();
-            HS_TICK(3);
-            const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3, sk0 = k0 >> 3;
-            const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;
-            const int nxs = nsx - (sk1 - sk0), tot = nxs + nsw;
-            for (int s = tid >> 5; s < tot; s += HS_NT / 32) {
-                cplx *Cg = W; int col0 = (s - nxs) * 8, ncols = nc;
-                if (s < nxs) { Cg = X; col0 = (s < sk0 ? s : s + (sk1 - sk0)) * 8; ncols = n; }
-                if (bw == HS_B) hs_strip_update<HS_RG, true>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw);
-                else hs_strip_update<HS_RG, false>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw);
-            }
-            __syncthreads();
-            HS_TICK(4);
-            continue;
-        }
-        // chunk list: matrix chunks except the panel's own, then the propagator chunks
-        const int skip = k0 / HS_B, total = nchm - 1 + ncha;
-        const int kmax = (bw + 3) & ~3;
-        auto chunk = [&](int q, cplx *&base, int &col0, int &ncols) {
-            if (q < nchm - 1) { const int j = q < skip ? q : q + 1; base = X; col0 = j * HS_B; ncols = n; }
-            else { base = W; col0 = (q - (nchm - 1)) * HS_B; ncols = nc; }
-        };
-        // software pipeline over half-tiles (16 columns): while one half is on the tensor pipe the other half's
-        // C fragments are in flight from L2; R of chunk q+1 is staged while chunk q computes.
-        cplx *base = nullptr, *bnext = nullptr; int col0 = 0, ncols = 0, c2 = 0, n2 = 0;
-        const bool active = (threadIdx.x >> 5) * 16 < n;
-        HSHalf h0, h1;
-        if (total > 0) {
-            chunk(0, base, col0, ncols);
-            hs_stage_R(sm, 0, base, ld, col0, ncols, bw);
-            if (active) hs_half_load(h0, base, ld, n, col0, ncols);
-        }
+        __syncthreads();
         HS_TICK(3);
-        for (int q = 0; q < total; q++) {
-            if (active) hs_half_load(h1, base, ld, n, col0 + 16, ncols);
-            cp_async_wait<0>();
-            __syncthreads();
-            const bool more = q + 1 < total;
-            if (more) { chunk(q + 1, bnext, c2, n2); hs_stage_R(sm, (q + 1) & 1, bnext, ld, c2, n2, bw); }
-            if (active) {
-                hs_half_compute(h0, sm, q & 1, 0, kmax);
-                hs_half_store(h0, base, ld, n, col0, ncols);
-                if (more) hs_half_load(h0, bnext, ld, n, c2, n2);
-                hs_half_compute(h1, sm, q & 1, 16, kmax);
-                hs_half_store(h1, base, ld, n, col0 + 16, ncols);
-            }
-            base = bnext; col0 = c2; ncols = n2;
+        // strip list: the 8-column strips of X except the panel's own four, then the strips of W; warp w takes
+        // strips w, w + 8, ...
+        const int sk0 = k0 >> 3;
+        const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;
+        const int nxs = nsx - (sk1 - sk0), tot = nxs + nsw;
+        for (int s = tid >> 5; s < tot; s += HS_NT / 32) {
+            const bool isx = s < nxs;
+            cplx *Cg = isx ? X : W;
+            const int col0 = (isx ? (s < sk0 ? s : s + (sk1 - sk0)) : s - nxs) * 8, ncols = isx ? n : nc;
+            if (tf) {
+                // (first panel of an in-place half-step: always 32 wide unless n < 32)
+                if (isx) hs_strip_update<HS_RG, false, 1>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+                else hs_strip_update<HS_RG, false, 2>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+            } else if (bw == HS_B) hs_strip_update<HS_RG, true, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+            else hs_strip_update<HS_RG, false, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
         }
         __syncthreads();
         HS_TICK(4);
@@ -602,12 +557,12 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
 }
 
 // ---- assembly of A (into Xn) and of W = C P_prev (into Wn) for half-step (i, kind) -------------------------
-// g_prev[k][m] = Xp[perm_prev[k]][pinv_prev[m]], P_prev[k][:] = Wp[perm_prev[k]][:]; blocks of 32 output rows,
+// g_prev[k][m] = Xp[rmap[k]][cmap[m]], P_prev[k][:] = Wp[rmap[k]][:]; blocks of 16 output rows,
 // the physical rows they need staged in the (idle) panel buffer so that every L2 read is a full row.
 struct HSAsm {
     cplx *stage;                       // staging area of 2 (RB + 2) rows of HS_NMAX elements (the idle panel buffer)
     HSTab *tb;                         // per-row tables (alias the idle candidate buffers)
-    const int *perm_prev, *pinv_prev;  // row maps of the previous half-step
+    const int *rmap, *cmap;            // logical row / column of the previous result -> physical row / column
 };
 // PART 0: A and W by all NT threads; 1: the tables and A only (all NT threads; ends with a barrier); 2: W only, by the
 // wnt threads wtid = 0 .. wnt-1 (no barrier; needs the tables of PART 1)
@@ -659,12 +614,12 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         if (kind == 0) {
             const int m = mk[2 * r + par] ? 1 : 0;
             tb.ra[r] = (short)m; tb.rb[r] = -1;
-            tb.ca[r] = (short)(m ? sm.pinv_prev[r] : -1); tb.cb[r] = -1;
+            tb.ca[r] = (short)(m ? sm.cmap[r] : -1); tb.cb[r] = -1;
         } else {
             const int s0 = half_nbr(r, par, 0, M, hp), s1 = half_nbr(r, par, 1, M, hp);
             tb.ra[r] = (short)s0; tb.rb[r] = (short)s1;
-            tb.ca[r] = (short)(s0 >= 0 ? sm.pinv_prev[s0] : -1);
-            tb.cb[r] = (short)(s1 >= 0 ? sm.pinv_prev[s1] : -1);
+            tb.ca[r] = (short)(s0 >= 0 ? sm.cmap[s0] : -1);
+            tb.cb[r] = (short)(s1 >= 0 ? sm.cmap[s1] : -1);
         }
     }
     __syncthreads();
@@ -686,7 +641,7 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         cplx *dst = stage + area * AREA;
         for (int idx = tid; idx < nst * ld; idx += HS_NT) {
             const int sl = idx / ld, c = idx - sl * ld;
-            cp_async16(dst + sl * HS_NMAX + c, Xp + (long long)sm.perm_prev[slo + sl] * ld + c, 16);
+            cp_async16(dst + sl * HS_NMAX + c, Xp + (long long)sm.rmap[slo + sl] * ld + c, 16);
         }
         cp_async_commit();
     };
@@ -746,11 +701,11 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
                 const int r = idx / nc, c = idx - r * nc;
                 rr[k] = r; cc[k] = c;
                 if (kind == 0) {
-                    if (tb.ra[r]) va[k] = ldcg(Wp + (long long)sm.perm_prev[r] * ld + c);
+                    if (tb.ra[r]) va[k] = ldcg(Wp + (long long)sm.rmap[r] * ld + c);
                 } else {
                     const int ua = tb.ra[r], ub = tb.rb[r];
-                    if (ua >= 0) va[k] = ldcg(Wp + (long long)sm.perm_prev[ua] * ld + c);
-                    if (ub >= 0) vb[k] = ldcg(Wp + (long long)sm.perm_prev[ub] * ld + c);
+                    if (ua >= 0) va[k] = ldcg(Wp + (long long)sm.rmap[ua] * ld + c);
+                    if (ub >= 0) vb[k] = ldcg(Wp + (long long)sm.rmap[ub] * ld + c);
                 }
             }
         }
@@ -761,77 +716,89 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
     if (PART == 0) __syncthreads();          // the tables alias the pivot-search buffers
 }
 
-__device__ unsigned hs_sm_arrivals[256];
+// buffer (0 / 1) that half-step hs leaves its result in: half-step 0 (B_0, assembled from the lead) writes buffer 1, every
+// F half-step reads one buffer and writes the other, every later B half-step works in place
+__device__ __forceinline__ int hs_out_buf(int hs) { return (((hs + 1) >> 1) & 1) ^ 1; }
 
 // ---- the sweep: one CTA per matrix, half-steps [hs_begin, hs_end) ----------------------------------------
-template <int MODE>
 __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
 {
     extern __shared__ __align__(16) unsigned char hs_smem_raw[];
     HSmem &sm = *reinterpret_cast<HSmem *>(hs_smem_raw);
-    const int tid = threadIdx.x, M = a.M, ld = a.ldn, nc = M / 2;
+    const int tid = threadIdx.x, M = a.M, L = a.L, ld = a.ldn, nc = M / 2;
     const long long unit = (long long)a.unit0 + blockIdx.x;
     const int bl = (int)(unit % a.nb);
     const int hs_begin = a.hs_begin + (int)(unit / a.nb) * a.unit_len;
     const int hs_end = (hs_begin + a.unit_len < a.hs_end) ? hs_begin + a.unit_len : a.hs_end;
     if (hs_begin >= hs_end) return;
-    // The two CTAs of an SM start a launch together and do identical work, so their phases (assembly / panel
-    // factorisation = FP64 pipe nearly idle, updates = FP64 tensor pipe saturated) stay aligned and nothing overlaps.
-    // Every second CTA to arrive on an SM therefore waits `stagger` cycles (about half a panel period) once per launch.
-    if (a.stagger > 0) {
-        if (tid == 0) {
-            unsigned smid;
-            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-            const unsigned arrival = atomicAdd(&hs_sm_arrivals[smid & 255], 1u);
-            if (arrival & 1u) {
-                const long long t0 = clock64();
-                while (clock64() - t0 < a.stagger) __nanosleep(200);
-            }
-        }
-        __syncthreads();
-    }
     const long long xs = (long long)ld * ld;
-    cplx *Xb[2] = {a.X0 + bl * xs, a.X1 + bl * xs};
-    cplx *Wb[2] = {a.P0 + bl * xs, a.P1 + bl * xs};
-    int *gperm = a.perm + (long long)bl * HS_NMAX;
+    cplx *const X0 = a.X0 + bl * xs, *const X1 = a.X1 + bl * xs, *const W0 = a.P0 + bl * xs, *const W1 = a.P1 + bl * xs;
+    int *gmaps = a.perm + (long long)bl * 2 * HS_NMAX;
     int *status_slot = a.status + bl;
     if (hs_begin > 0) {
-        if (tid < HS_NMAX) sm.perm[tid] = gperm[tid];
-        __syncthreads();
-        const int hp_ = hs_begin - 1, ip = hp_ >> 1, kp = hp_ & 1;
-        const int np = half_count(M, kp == 0 ? ((ip + 1) & 1) : (ip & 1));
-        if (tid < np) sm.pinv[sm.perm[tid]] = tid;
+        if (tid < HS_NMAX) { sm.rmap[tid] = gmaps[tid]; sm.cmap[tid] = gmaps[HS_NMAX + tid]; }
         __syncthreads();
     }
     if (tid < 16) sm.prof[tid] = 0;
+    const int bz = a.bz0 + bl, dev = bz / a.n_E;
+    const double E = a.energies[bz % a.n_E];
+    const HSXf xf = {sm.xf_sr, sm.xf_sw, sm.xf_dre, sm.xf_mc, sm.xf_dcol, a.eta};
     int n = 0;
     for (int hs = hs_begin; hs < hs_end; hs++) {
-        const int i = hs >> 1, kind = hs & 1, cur = hs & 1;
-        if (tid < HS_NMAX) { sm.perm_prev[tid] = sm.perm[tid]; sm.pinv_prev[tid] = sm.pinv[tid]; }
+        const int i = hs >> 1, kind = hs & 1;
+        const int ob = hs_out_buf(hs), ib = hs > 0 ? hs_out_buf(hs - 1) : 0;
+        cplx *Xn = ob ? X1 : X0, *Wn = ob ? W1 : W0;
+        const cplx *Xp = ib ? X1 : X0, *Wp = ib ? W1 : W0;
+        const bool inplace = kind == 0 && hs > 0;
+        const int par = kind == 0 ? ((i + 1) & 1) : (i & 1);
+        n = half_count(M, par);
+        if (tid < HS_NMAX) { sm.rmap_prev[tid] = sm.rmap[tid]; sm.cmap_prev[tid] = sm.cmap[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
-        static_assert(2 * (16 + 2) * HS_NMAX <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
-        const HSAsm av = {sm.panel, reinterpret_cast<HSTab *>(sm.crow), sm.perm_prev, sm.pinv_prev};
-        hs_assemble<HS_NT, 16>(av, a, bl, i, kind, hs == 0, Xb[cur], Wb[cur], Xb[cur ^ 1], Wb[cur ^ 1]);
+        if (inplace) {
+            // tables of the in-place assembly (HSXf): atom r of this B half sits in physical row rmap[r] and its column
+            // in physical column cmap[r] of the previous (F) result
+            if (tid < n) {
+                const int r = tid, j = 2 * r + par, rho = sm.rmap_prev[r], gam = sm.cmap_prev[r];
+                const double m = a.bond[((long long)dev * (L + 1) + i) * M + j] ? 1.0 : 0.0;      // m'_{i-1}
+                sm.xf_sr[rho] = -a.t * a.t * m; sm.xf_sw[rho] = a.t * m;
+                sm.xf_dre[rho] = E - a.onsite[((long long)dev * L + i) * M + j];
+                sm.xf_dcol[rho] = (short)gam;
+                sm.xf_mc[gam] = m;
+            }
+        } else {
+            static_assert(2 * (16 + 2) * HS_NMAX <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
+            const HSAsm av = {sm.panel, reinterpret_cast<HSTab *>(sm.crow), sm.rmap_prev, sm.cmap_prev};
+            hs_assemble<HS_NT, 16>(av, a, bl, i, kind, hs == 0, Xp, Wp, Xn, Wn);
+        }
         __syncthreads();
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
-        n = half_count(M, kind == 0 ? ((i + 1) & 1) : (i & 1));
-        hs_gauss_jordan<MODE>(sm, Xb[cur ^ 1], Wb[cur ^ 1], ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr);
+        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr, inplace, xf);
+        // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
+        // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
+        // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].
+        if (tid < n) {
+            const int g0 = inplace ? sm.cmap_prev[tid] : tid, r0 = inplace ? sm.rmap_prev[tid] : tid;
+            sm.rmap[tid] = sm.perm[g0];
+            sm.cmap[tid] = sm.pinv[r0];
+        }
+        __syncthreads();
     }
-    if (tid < HS_NMAX) gperm[tid] = sm.perm[tid];
+    if (tid < HS_NMAX) { gmaps[tid] = sm.rmap[tid]; gmaps[HS_NMAX + tid] = sm.cmap[tid]; }
     if (a.prof && tid < 16) a.prof[bl * 16 + tid] += sm.prof[tid];
     if (hs_end == a.hs_end && (a.g_out || a.P_out)) {
-        const int fin = hs_end & 1;                  // buffer written by the last half-step
+        const int fb = hs_out_buf(hs_end - 1);
+        const cplx *Xf = fb ? X1 : X0, *Wf = fb ? W1 : W0;
         const long long os = (long long)a.nh * a.nh;
         if (a.g_out)
             for (int idx = tid; idx < n * n; idx += HS_NT) {
                 const int k = idx / n, m = idx % n;
-                a.g_out[bl * os + idx] = ldcg(Xb[fin] + (long long)sm.perm[k] * ld + sm.pinv[m]);
+                a.g_out[bl * os + idx] = ldcg(Xf + (long long)sm.rmap[k] * ld + sm.cmap[m]);
             }
         if (a.P_out)
             for (int idx = tid; idx < n * nc; idx += HS_NT) {
                 const int k = idx / nc, c = idx % nc;
-                a.P_out[bl * os + (long long)k * a.nh + c] = ldcg(Wb[fin] + (long long)sm.perm[k] * ld + c);
+                a.P_out[bl * os + (long long)k * a.nh + c] = ldcg(Wf + (long long)sm.rmap[k] * ld + c);
             }
     }
 }

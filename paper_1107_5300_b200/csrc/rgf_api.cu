@@ -22,7 +22,6 @@
 #include "gj_inverse32.cuh"
 #include "half_kernels.cuh"
 #include "half_sweep.cuh"
-#include "half_sweep_la.cuh"
 #include "half_sweep_c64.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
@@ -130,9 +129,7 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<4>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
-    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
-    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
-    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_la_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmemLA)));
+    CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
     CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_c64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HC64Smem)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_unpermute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024));
     p->attrs_set = true;
@@ -540,7 +537,7 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
     const size_t xb = sizeof(cplx) * (size_t)a.ldn * a.ldn * nb;
     Buf *bufs[] = {&w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1};
     for (Buf *b : bufs) if ((rc = ensure(p, *b, xb))) return rc;
-    if ((rc = ensure(p, w.Fperm, sizeof(int) * (size_t)HS_NMAX * nb))) return rc;
+    if ((rc = ensure(p, w.Fperm, sizeof(int) * 2 * (size_t)HS_NMAX * nb))) return rc;      // row and column maps
     a.nb = nb;
     a.X0 = ptr<cplx>(w.Fx0); a.X1 = ptr<cplx>(w.Fx1); a.P0 = ptr<cplx>(w.Fp0); a.P1 = ptr<cplx>(w.Fp1);
     a.perm = ptr<int>(w.Fperm);
@@ -556,13 +553,7 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
     // (nb > slots) and stream order is the only dependency.
     int sms = 0, occ = 0;
     CUDA_TRY(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
-    static const int hs_mode = getenv("RGF_HS_MODE") ? atoi(getenv("RGF_HS_MODE")) : 1;     // 0: chunk updates with staged R (round-1 kernel), 1: barrier-free strips
-    void (*kern)(HSweepArgs) = hs_mode == 0 ? half_sweep_kernel<0> : hs_mode == 1 ? half_sweep_kernel<1> : half_sweep_la_kernel;
-    const int kern_nt = hs_mode == 2 ? LA_NT : HS_NT;
-    const size_t kern_smem = hs_mode == 2 ? sizeof(HSmemLA) : sizeof(HSmem);
-    static const int hs_stagger = getenv("RGF_HS_STAGGER") ? atoi(getenv("RGF_HS_STAGGER")) : 0;
-    a.stagger = hs_stagger;
-    CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kern_nt, kern_smem));
+    CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, half_sweep_kernel, HS_NT, sizeof(HSmem)));
     int slots = std::max(1, occ) * sms;
     if (p->cohort_override > 0) slots = std::min(slots, p->cohort_override);      // rgf_set_cohort: fewer units per launch
     const bool timed = p->profiling > 0 && p->in_sweep;
@@ -573,7 +564,7 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
             if (rc2) return rc2;
             CUDA_TRY(p, cudaEventRecord(e0, w.stream));
         }
-        kern<<<grid, kern_nt, kern_smem, w.stream>>>(a);
+        half_sweep_kernel<<<grid, HS_NT, sizeof(HSmem), w.stream>>>(a);
         if (timed) CUDA_TRY(p, cudaEventRecord(e1, w.stream));
         p->stats.launches++;
         if (p->in_sweep) p->stats.launches_inverse_update++;
