@@ -62,7 +62,7 @@ struct HSmem {
     int prow[HS_B];
     // in-place assembly of a kind-B half-step (HSXf), per physical row / column of the previous result
     double xf_sr[HS_NMAX], xf_sw[HS_NMAX], xf_dre[HS_NMAX], xf_mc[HS_NMAX];
-    short xf_dcol[HS_NMAX];
+    short xf_dcol[HS_NMAX], xf_pa[HS_NMAX], xf_pb[HS_NMAX];
     long long prof[16];          // per-phase cycle counters of thread 0 (debugging aid, RGF_HS_PROF)
 };
 
@@ -354,8 +354,13 @@ struct HSXf {
     const double *sr, *sw, *dre, *mc;
     const short *dcol;
     double eta;
+    // kind-F half-steps: W = C P_prev is a two-row stencil of the previous propagator (other buffer), W[r] = t (Wp[pa[r]] +
+    // Wp[pb[r]]), pa / pb = physical rows of the lower / upper B neighbour or -1; also formed by whoever loads first
+    const cplx *Wp;
+    const short *pa, *pb;
+    double t;
 };
-// TF: 0 = plain load, 1 = element of X, 2 = element of W
+// TF: 0 = plain load, 1 = element of X (kind B), 2 = element of W (kind B), 3 = W of a kind-F half-step (hs_wf_load)
 template <int TF>
 __device__ __forceinline__ cplx hs_xf(const HSXf &xf, cplx v, int rho, int gamma)
 {
@@ -368,6 +373,24 @@ __device__ __forceinline__ cplx hs_xf(const HSXf &xf, cplx v, int rho, int gamma
         v.x *= sc; v.y *= sc;
     }
     return v;
+}
+
+// two adjacent elements (row r, columns gamma0, gamma0 + 1; gamma0 even) of W = C P_prev
+__device__ __forceinline__ void hs_wf_load2(const HSXf &xf, int ld, int r, int gamma0, double &a0, double &a1, double &a2, double &a3)
+{
+    const int pa = xf.pa[r], pb = xf.pb[r];
+    double b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0, c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+    if (pa >= 0) ld256cg(xf.Wp + (long long)pa * ld + gamma0, b0, b1, b2, b3);
+    if (pb >= 0) ld256cg(xf.Wp + (long long)pb * ld + gamma0, c0, c1, c2, c3);
+    a0 = xf.t * (b0 + c0); a1 = xf.t * (b1 + c1); a2 = xf.t * (b2 + c2); a3 = xf.t * (b3 + c3);
+}
+__device__ __forceinline__ cplx hs_wf_load1(const HSXf &xf, int ld, int r, int gamma)
+{
+    const int pa = xf.pa[r], pb = xf.pb[r];
+    cplx va = cmake(0.0, 0.0), vb = cmake(0.0, 0.0);
+    if (pa >= 0) va = ldcg(xf.Wp + (long long)pa * ld + gamma);
+    if (pb >= 0) vb = ldcg(xf.Wp + (long long)pb * ld + gamma);
+    return cmake(xf.t * (va.x + vb.x), xf.t * (va.y + vb.y));
 }
 
 // ---- barrier-free update of one 8-column strip: C[:, col0 .. col0+8) += Mult (n x 32, sm.panel) * R ---------------
@@ -388,8 +411,9 @@ __device__ __forceinline__ void hs_acc_load(HSAcc<RG> &h, const cplx *Cl, int ld
         double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
         if (rr < n && cok) {
             // elements (rr, c) and (rr, c + 1), c even: one 32-byte sector, one LDG.256.  c + 1 may be the padding column.
-            ld256cg(Cl + (long long)rr * ld, a0, a1, a2, a3);
-            if (TF) {
+            if (TF == 3) hs_wf_load2(xf, ld, rr, gamma0, a0, a1, a2, a3);
+            else ld256cg(Cl + (long long)rr * ld, a0, a1, a2, a3);
+            if (TF == 1 || TF == 2) {
                 const cplx v0 = hs_xf<TF>(xf, cmake(a0, a1), rr, gamma0), v1 = hs_xf<TF>(xf, cmake(a2, a3), rr, gamma0 + 1);
                 a0 = v0.x; a1 = v0.y; a2 = v1.x; a3 = v1.y;
             }
@@ -456,7 +480,8 @@ __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *pr
             bb[q] = cmake(0.0, 0.0);
             if (k < bw && colok) {
                 const int rho = prow[k];
-                bb[q] = hs_xf<TF>(xf, ldcg(Cg + (long long)rho * ld + col0 + g), rho, col0 + g);
+                if (TF == 3) bb[q] = hs_wf_load1(xf, ld, rho, col0 + g);
+                else bb[q] = hs_xf<TF>(xf, ldcg(Cg + (long long)rho * ld + col0 + g), rho, col0 + g);
             }
         }
     }
@@ -479,10 +504,11 @@ __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *pr
     }
 }
 
-// ---- [X | W] <- A^-1 [I | W] in place (X holds A on entry, or, with inplace, the previous result that HSXf turns
-// into [A | W] while panel 0 is loaded and applied); fills sm.perm / sm.pinv ---------------------------------------
+// ---- [X | W] <- A^-1 [I | W] in place; fills sm.perm / sm.pinv.  X holds A on entry (xtf = 0) or the previous result
+// that HSXf turns into A while panel 0 is loaded and applied (xtf = 1); W likewise: wtf = 0 (W in place), 2 (previous
+// propagator, scaled in place) or 3 (stencil of the previous propagator in the other buffer) ---------------------------------------
 __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof,
-                                                bool inplace, const HSXf &xf)
+                                                int xtf, int wtf, const HSXf &xf)
 {
     long long tc = prof ? clock64() : 0;
 #define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
@@ -493,8 +519,8 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
     const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3;
     for (int k0 = 0; k0 < n; k0 += HS_B) {
         const int bw = (n - k0 < HS_B) ? (n - k0) : HS_B;
-        const bool tf = inplace && k0 == 0;
-        if (!tf) {
+        const bool tf = (xtf | wtf) != 0 && k0 == 0;
+        if (!(tf && xtf)) {
             for (int e = tid; e < HS_NMAX * HS_B; e += HS_NT) {
                 const int rr = e / HS_B, c = e % HS_B;
                 const bool ok = rr < n && c < bw;
@@ -543,10 +569,12 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
             const bool isx = s < nxs;
             cplx *Cg = isx ? X : W;
             const int col0 = (isx ? (s < sk0 ? s : s + (sk1 - sk0)) : s - nxs) * 8, ncols = isx ? n : nc;
-            if (tf) {
-                // (first panel of an in-place half-step: always 32 wide unless n < 32)
-                if (isx) hs_strip_update<HS_RG, false, 1>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
-                else hs_strip_update<HS_RG, false, 2>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+            const int tfs = tf ? (isx ? xtf : wtf) : 0;
+            if (tfs) {
+                // (first panel: always 32 wide unless n < 32)
+                if (tfs == 1) hs_strip_update<HS_RG, false, 1>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+                else if (tfs == 2) hs_strip_update<HS_RG, false, 2>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+                else hs_strip_update<HS_RG, false, 3>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
             } else if (bw == HS_B) hs_strip_update<HS_RG, true, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
             else hs_strip_update<HS_RG, false, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
         }
@@ -742,7 +770,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
     if (tid < 16) sm.prof[tid] = 0;
     const int bz = a.bz0 + bl, dev = bz / a.n_E;
     const double E = a.energies[bz % a.n_E];
-    const HSXf xf = {sm.xf_sr, sm.xf_sw, sm.xf_dre, sm.xf_mc, sm.xf_dcol, a.eta};
+    HSXf xf = {sm.xf_sr, sm.xf_sw, sm.xf_dre, sm.xf_mc, sm.xf_dcol, a.eta, nullptr, sm.xf_pa, sm.xf_pb, a.t};
     int n = 0;
     for (int hs = hs_begin; hs < hs_end; hs++) {
         const int i = hs >> 1, kind = hs & 1;
@@ -769,11 +797,23 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         } else {
             static_assert(2 * (16 + 2) * HS_NMAX <= HS_NMAX * HS_LDP, "two staging areas must fit in the panel buffer");
             const HSAsm av = {sm.panel, reinterpret_cast<HSTab *>(sm.crow), sm.rmap_prev, sm.cmap_prev};
-            hs_assemble<HS_NT, 16>(av, a, bl, i, kind, hs == 0, Xp, Wp, Xn, Wn);
+            if (hs == 0) hs_assemble<HS_NT, 16, 0>(av, a, bl, i, kind, true, Xp, Wp, Xn, Wn);
+            else {
+                // kind F: A is gathered through shared memory; W = C P_prev is left to the first panel's strips
+                if (tid < n) {
+                    const uint8_t *hp = a.hop + ((long long)dev * L + i) * M;
+                    const int s0 = half_nbr(tid, par, 0, M, hp), s1 = half_nbr(tid, par, 1, M, hp);
+                    sm.xf_pa[tid] = (short)(s0 >= 0 ? sm.rmap_prev[s0] : -1);
+                    sm.xf_pb[tid] = (short)(s1 >= 0 ? sm.rmap_prev[s1] : -1);
+                }
+                hs_assemble<HS_NT, 16, 1>(av, a, bl, i, kind, false, Xp, Wp, Xn, Wn);
+            }
         }
         __syncthreads();
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
-        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr, inplace, xf);
+        xf.Wp = Wp;
+        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr,
+                        inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf);
         // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
         // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
         // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].
