@@ -3,20 +3,27 @@
 //
 // One CTA owns one (device, energy) pair and runs its half-steps back to back (Eq. 4-5
 // on the slicing B_0, F_0, B_1, F_1, ...; half_kernels.cuh states the recursion):
-//     A = z - eps - C g_prev C^T  [- Sigma_L/R at the ends]         assembly, O(n^2), staged through smem
+//     A = z - eps - C g_prev C^T  [- Sigma_L/R at the ends]         assembly, O(n^2)
 //     [ g | P ] = A^-1 [ I | C P_prev ]                            ONE in-place Gauss-Jordan on the augmented matrix
 // The propagator columns ride along as extra right-hand sides of the elimination, so inverse (8 n^3)
 // and propagator product (8 n^3 real flops) are the same kernel loop: for every panel of 32 columns
 //     1. the n x 32 panel is factored in shared memory with partial pivoting (rows never move; thread = row;
 //        8-column sub-blocks in registers, the other panel columns by DMMA),
-//     2. every other 32-column chunk of [X | W] is updated in place, C += Mult * R on the FP64 tensor
-//        pipe (mma.sync m8n8k4 = DMMA.8x8x4), Mult read from the factored panel in shared memory, the
-//        32 pivot rows R staged by cp.async, C fragments straight from / to L2.
-// Rows are never exchanged: with p_k the pivot row of column k the result sits at
-//     g[k][p_c] = X[p_k][c],   P[k][:] = W[p_k][:]
-// and the next half-step reads it through the maps perm[k] = p_k, pinv[p_k] = k (no unpermute pass).
-// State per matrix in HBM/L2: X (2 buffers), W (2 buffers), perm.  2 CTAs per SM (113 KB of shared
-// memory each, <= 128 registers) so that one CTA's latency-bound pivot search overlaps the other's DMMAs.
+//     2. every other 8-column strip of [X | W] is updated in place, C += Mult * R on the FP64 tensor pipe
+//        (mma.sync m8n8k4 = DMMA.8x8x4): a warp owns a strip, snapshots the strip's 32 pivot rows R in its B
+//        fragments, reads Mult from the factored panel in shared memory and streams the C fragments L2 ->
+//        registers -> L2 (no barrier and no shared-memory staging between the warps of an update).
+// Rows are never exchanged: with p_k the pivot row of column k the result of an elimination sits at
+//     (A^-1)[k][p_c] = X[p_k][c],   (A^-1 W)[k][:] = W[p_k][:]
+// and the next half-step reads it through row / column maps (no unpermute pass).
+// Assembly is mostly not a pass of its own:
+//     kind B  A_B = z - eps - t^2 m' (.) gF_prev (.) m', W_B = t m' (.) PF_prev are the previous result scaled element by
+//             element (+ a diagonal): left in place, in its permuted order, and transformed by whoever loads an element
+//             first (panel 0 and its strips), HSXf;
+//     kind F  A_F = z - eps - C gB C^T is a 2 x 2 stencil in rows and columns: gathered through shared memory
+//             (hs_assemble); W_F = C PB is a two-row stencil, formed by the first panel's strips from the other buffer.
+// State per matrix in HBM/L2: X (2 buffers), W (2 buffers), the two maps.  2 CTAs per SM (87 KB of shared memory each,
+// 128 registers) so that one CTA's latency-bound pivot chain overlaps the other's DMMAs.
 #pragma once
 #include "half_kernels.cuh"
 #include "rgf_common.cuh"
@@ -26,7 +33,7 @@ namespace rgf {
 constexpr int HS_NT = 256, HS_NMAX = 128, HS_B = 32, HS_SB = 8;
 constexpr int HS_LDP = HS_B + 4;        // 36: A-fragment reads of the panel conflict-free
 constexpr int HS_LDR = HS_B + 2;        // 34: B-fragment reads conflict-free
-constexpr int HS_STAGE_ROWS = 36;
+constexpr int HS_TRACE = 1024;
 #ifndef HS_FSB
 #define HS_FSB 8                        // sub-block width of the panel factorisation
 #endif
@@ -41,12 +48,13 @@ struct HSweepArgs {
     const uint8_t *bond, *hop;
     const cplx *gL, *gR;
     cplx *X0, *X1, *P0, *P1;      // [nb][ldn*ldn] each
-    int *perm;                    // [nb][HS_NMAX]
+    int *perm;                    // [nb][2][HS_NMAX]: row and column maps of a matrix between launches
     int *status;                  // [nb]
     int hs_begin, hs_end;         // half-steps [begin, end) of the whole sweep: hs = 2 i + kind
     int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
                                   // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
     long long *prof;              // optional [nb][16] cycle counters of thread 0 per phase (NULL = off)
+    long long *trace;             // optional [nb][HS_TRACE] event log of thread 0: [0] = SM id, then (globaltimer ns << 8 | event)
     cplx *g_out, *P_out;          // after half-step hs_end - 1: g dense n x n (ld n) and P (ld nh), stride nh*nh; may be NULL
 };
 
@@ -508,8 +516,9 @@ __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *pr
 // that HSXf turns into A while panel 0 is loaded and applied (xtf = 1); W likewise: wtf = 0 (W in place), 2 (previous
 // propagator, scaled in place) or 3 (stencil of the previous propagator in the other buffer) ---------------------------------------
 __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof,
-                                                int xtf, int wtf, const HSXf &xf)
+                                                int xtf, int wtf, const HSXf &xf, long long *trace, int &tri)
 {
+#define HS_EV(id) do { if (trace && threadIdx.x == 0 && tri < HS_TRACE) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); trace[tri++] = (long long)((t_ << 8) | (unsigned)(id)); } } while (0)
     long long tc = prof ? clock64() : 0;
 #define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
     const int tid = threadIdx.x;
@@ -549,6 +558,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         }
         __syncthreads();
         HS_TICK(1);
+        HS_EV(1);
         hs_factor_panel<HS_FSB>(view, grp, n, k0, bw, used, status_slot);
         HS_TICK(2);
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
@@ -560,6 +570,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
         __syncthreads();
         HS_TICK(3);
+        HS_EV(2);
         // strip list: the 8-column strips of X except the panel's own four, then the strips of W; warp w takes
         // strips w, w + 8, ...
         const int sk0 = k0 >> 3;
@@ -570,18 +581,23 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
             cplx *Cg = isx ? X : W;
             const int col0 = (isx ? (s < sk0 ? s : s + (sk1 - sk0)) : s - nxs) * 8, ncols = isx ? n : nc;
             const int tfs = tf ? (isx ? xtf : wtf) : 0;
-            if (tfs) {
-                // (first panel: always 32 wide unless n < 32)
-                if (tfs == 1) hs_strip_update<HS_RG, false, 1>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
-                else if (tfs == 2) hs_strip_update<HS_RG, false, 2>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
-                else hs_strip_update<HS_RG, false, 3>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
-            } else if (bw == HS_B) hs_strip_update<HS_RG, true, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
-            else hs_strip_update<HS_RG, false, 0>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf);
+            // FULL = straight-line code over all eight k-steps: Mult columns / pivot rows beyond the panel width are zero,
+            // so a slightly narrow panel (n = 122: the last one is 26 wide) only adds DMMAs on zeros
+            const bool full = bw > HS_B - 12;
+#define HS_STRIP(F, T) hs_strip_update<HS_RG, F, T>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf)
+            if (full) {
+                if (tfs == 0) HS_STRIP(true, 0); else if (tfs == 1) HS_STRIP(true, 1); else if (tfs == 2) HS_STRIP(true, 2); else HS_STRIP(true, 3);
+            } else {
+                if (tfs == 0) HS_STRIP(false, 0); else if (tfs == 1) HS_STRIP(false, 1); else if (tfs == 2) HS_STRIP(false, 2); else HS_STRIP(false, 3);
+            }
+#undef HS_STRIP
         }
         __syncthreads();
         HS_TICK(4);
+        HS_EV(3);
     }
 #undef HS_TICK
+#undef HS_EV
 }
 
 // ---- assembly of A (into Xn) and of W = C P_prev (into Wn) for half-step (i, kind) -------------------------
@@ -768,6 +784,9 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         __syncthreads();
     }
     if (tid < 16) sm.prof[tid] = 0;
+    long long *trace = a.trace ? a.trace + (long long)bl * HS_TRACE : nullptr;
+    int tri = 1;
+    if (trace && tid == 0) { unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); trace[0] = smid; }
     const int bz = a.bz0 + bl, dev = bz / a.n_E;
     const double E = a.energies[bz % a.n_E];
     HSXf xf = {sm.xf_sr, sm.xf_sw, sm.xf_dre, sm.xf_mc, sm.xf_dcol, a.eta, nullptr, sm.xf_pa, sm.xf_pb, a.t};
@@ -783,6 +802,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         if (tid < HS_NMAX) { sm.rmap_prev[tid] = sm.rmap[tid]; sm.cmap_prev[tid] = sm.cmap[tid]; }
         __syncthreads();
         long long tc0 = a.prof ? clock64() : 0;
+        if (trace && tid == 0 && tri < HS_TRACE) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); trace[tri++] = (long long)((t_ << 8) | 0u); }
         if (inplace) {
             // tables of the in-place assembly (HSXf): atom r of this B half sits in physical row rmap[r] and its column
             // in physical column cmap[r] of the previous (F) result
@@ -813,7 +833,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         xf.Wp = Wp;
         hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr,
-                        inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf);
+                        inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf, trace, tri);
         // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
         // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
         // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].

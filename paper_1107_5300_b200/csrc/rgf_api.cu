@@ -542,10 +542,12 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
     a.X0 = ptr<cplx>(w.Fx0); a.X1 = ptr<cplx>(w.Fx1); a.P0 = ptr<cplx>(w.Fp0); a.P1 = ptr<cplx>(w.Fp1);
     a.perm = ptr<int>(w.Fperm);
     static const bool prof_on = getenv("RGF_HS_PROF") != nullptr;          // debugging aid: per-phase cycle counters
+    static const char *trace_path = getenv("RGF_HS_TRACE");                // debugging aid: event log of the first launch
     if (prof_on) {
-        if ((rc = ensure(p, p->counters, sizeof(long long) * 16 * (size_t)nb))) return rc;
-        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * 16 * (size_t)nb, w.stream));
+        if ((rc = ensure(p, p->counters, sizeof(long long) * (16 + HS_TRACE) * (size_t)nb))) return rc;
+        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * (16 + HS_TRACE) * (size_t)nb, w.stream));
         a.prof = ptr<long long>(p->counters);
+        if (trace_path) a.trace = a.prof + 16 * (size_t)nb;
     }
     // Rounds of units: with more matrices than resident CTA slots (2 per SM) a single launch would run 512 matrices
     // as 296 + 216, the second wave half empty.  Instead every launch runs `slots` units of unit_len half-steps; unit
@@ -586,11 +588,23 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
         std::vector<long long> h(16 * (size_t)nb);
         CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->counters.p, sizeof(long long) * h.size(), cudaMemcpyDeviceToHost, w.stream));
         CUDA_TRY(p, cudaStreamSynchronize(w.stream));
+        if (trace_path) {
+            std::vector<long long> tr((size_t)HS_TRACE * nb);
+            CUDA_TRY(p, cudaMemcpy(tr.data(), a.trace, sizeof(long long) * tr.size(), cudaMemcpyDeviceToHost));
+            if (FILE *f = fopen(trace_path, "w")) {
+                for (int b = 0; b < nb; b++) {
+                    fprintf(f, "%d %lld", b, tr[(size_t)b * HS_TRACE]);
+                    for (int k = 1; k < HS_TRACE && tr[(size_t)b * HS_TRACE + k]; k++) fprintf(f, " %lld", tr[(size_t)b * HS_TRACE + k]);
+                    fprintf(f, "\n");
+                }
+                fclose(f);
+            }
+        }
         double s[16] = {0};
         for (int b = 0; b < nb; b++) for (int k = 0; k < 16; k++) s[k] += (double)h[16 * (size_t)b + k];
         const double hsn = (double)nb * a.hs_end;
-        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           slots 8-15: %.0f %.0f %.0f %.0f %.0f %.0f %.0f %.0f   slots 5-7: %.0f %.0f %.0f\n",
-                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[8] / hsn, s[9] / hsn, s[10] / hsn, s[11] / hsn, s[12] / hsn, s[13] / hsn, s[14] / hsn, s[15] / hsn, s[5] / hsn, s[6] / hsn, s[7] / hsn);
+        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           in-panel: pivot-row snapshot %.0f  DMMA %.0f\n",
+                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[13] / hsn, s[14] / hsn);
     }
     return RGF_OK;
 }
