@@ -576,10 +576,15 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         const int sk0 = k0 >> 3;
         const int sk1 = (sk0 + HS_B / 8 < nsx) ? sk0 + HS_B / 8 : nsx;
         const int nxs = nsx - (sk1 - sk0), tot = nxs + nsw;
-        for (int s = tid >> 5; s < tot; s += HS_NT / 32) {
+        auto strip_of = [&](int s, cplx *&Cg, int &col0, int &ncols) {
             const bool isx = s < nxs;
-            cplx *Cg = isx ? X : W;
-            const int col0 = (isx ? (s < sk0 ? s : s + (sk1 - sk0)) : s - nxs) * 8, ncols = isx ? n : nc;
+            Cg = isx ? X : W;
+            col0 = (isx ? (s < sk0 ? s : s + (sk1 - sk0)) : s - nxs) * 8; ncols = isx ? n : nc;
+            return isx;
+        };
+        for (int s = tid >> 5; s < tot; s += HS_NT / 32) {
+            cplx *Cg; int col0, ncols;
+            const bool isx = strip_of(s, Cg, col0, ncols);
             const int tfs = tf ? (isx ? xtf : wtf) : 0;
             // FULL = straight-line code over all eight k-steps: Mult columns / pivot rows beyond the panel width are zero,
             // so a slightly narrow panel (n = 122: the last one is 26 wide) only adds DMMAs on zeros
@@ -683,10 +688,11 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         int slo, nst;
         rows_of(r0, slo, nst);
         cplx *dst = stage + area * AREA;
-        for (int idx = tid; idx < nst * ld; idx += HS_NT) {
-            const int sl = idx / ld, c = idx - sl * ld;
-            cp_async16(dst + sl * HS_NMAX + c, Xp + (long long)sm.rmap[slo + sl] * ld + c, 16);
-        }
+        // thread = (row tid / 128 + k NT / 128, column tid % 128): no division by the runtime ld
+        const int c = tid & (HS_NMAX - 1);
+        if (c < ld)
+            for (int sl = tid / HS_NMAX; sl < nst; sl += HS_NT / HS_NMAX)
+                cp_async16(dst + sl * HS_NMAX + c, Xp + (long long)sm.rmap[slo + sl] * ld + c, 16);
         cp_async_commit();
     };
     stage_rows(0, 0);
@@ -698,11 +704,12 @@ __device__ __forceinline__ void hs_assemble(const HSAsm &sm, const HSweepArgs &a
         else cp_async_wait<0>();
         __syncthreads();
         const cplx *st = stage + (blk & 1) * AREA;
-        for (int idx = tid; idx < (r1 - r0) * n; idx += HS_NT) {
-            const int rl = idx / n, c = idx - rl * n, r = r0 + rl;
+        const int c = tid & (HS_NMAX - 1);
+        const int ca = c < n ? tb.ca[c] : -1, cb = c < n ? tb.cb[c] : -1;
+        if (c < n)
+        for (int r = r0 + tid / HS_NMAX; r < r1; r += HS_NT / HS_NMAX) {
             cplx v = cmake(0.0, 0.0);
             if (r == c) v = cmake(tb.eps[r], a.eta);
-            const int ca = tb.ca[c], cb = tb.cb[c];
             double sx = 0.0, sy = 0.0;
             if (kind == 0) {
                 if (tb.ra[r] && ca >= 0) { const cplx g = st[(r - slo) * HS_NMAX + ca]; sx = g.x; sy = g.y; }
