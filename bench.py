@@ -11,7 +11,7 @@ Metric: RGF slice-steps/s (slice-step = one (seed, energy, slice) triple).
   value      inputs resident in HBM (energies / T_out are device tensors, ribbon already set)
   e2e        the same through the C ABI with HOST buffers: rgf_set_device(host onsite) +
              rgf_transmission(host energies -> host T) inside the timed region
-  roofline   dominant kernel = gj_update_kernel (FP64 DMMA): algorithmic flops per launch divided
+  roofline   dominant kernel = half_sweep_kernel (FP64 DMMA): algorithmic flops per launch divided
              by its mean CUDA-event duration inside the timed region, against the FP64 tensor
              ceiling measured live on the same GPU (rgf_fp64_peak_tflops)
   cpu_baseline  the oracle (oracle/rgf_oracle.c, naive LU, OpenMP over energies) on a bounded sample
@@ -36,7 +36,7 @@ from paper_1107_5300_b200 import inputs  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the headline launch configuration,
 # from the ncu --set full capture summarised in profiles/ (bytes; None = not captured for this formulation)
-TRAFFIC_NCU = {"half": 84.33e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
+TRAFFIC_NCU = {"half": 68.63e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
 
 METRIC = "rgf_slice_steps_per_s"
 UNIT = "slice-steps/s"
