@@ -270,6 +270,33 @@ def test_fused_kernel_unit_rounds(rgf, plan, oracle):
     assert plan.stats()["launches"] > 0
 
 
+def test_fused_state_across_unit_rounds_with_vacancies(rgf, plan, oracle):
+    """State (g, P) of the fused kernel after 35 slices = 70 half-steps, i.e. two units, with 2 CTA slots for 3 energies: the B
+    half-steps are assembled in place from the previous result through the row / column maps, which a matrix carries
+    through HBM from one launch to the next; odd width (the two halves differ in size) and vacancies (masked rows / columns
+    of the in-place assembly)."""
+    M, L, ns = 21, 40, 35
+    on = inputs.anderson(M, L, 0.3, 77)
+    vac = inputs.edge_vacancies(M, L, 0.25, 13)
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.array([-1.2, 0.31, 0.95])
+    plan.set_device(on, -2.7, vac)
+    rgf.rgf_set_cohort(plan.handle, 2)
+    g = np.empty((3, M, M), dtype=complex)
+    P = np.empty((3, M, M), dtype=complex)
+    rgf.rgf_sweep_state(plan.handle, 0, E, 3, 1e-9, rgf.RGF_C128, ns, g, P)
+    rgf.rgf_set_cohort(plan.handle, 0)
+    for k, e in enumerate(E):
+        g0, P0 = oracle.sweep_state(on, vac, -2.7, e, 1e-9, ns)
+        hg = ~np.isnan(g[k].real)
+        fr = (np.arange(M) % 2) == ((ns - 1) % 2)
+        assert np.array_equal(hg, np.outer(fr, fr))
+        assert np.max(np.abs(g[k][hg] - g0[hg])) < 1e-9 * np.max(np.abs(g0))
+        have = ~np.isnan(P[k].real)
+        assert np.array_equal(have, np.outer(fr, (np.arange(M) % 2) == 1))
+        assert np.max(np.abs(P[k][have] - P0[have])) < 1e-9 * max(1e-300, np.max(np.abs(P0)))
+
+
 @pytest.mark.parametrize("M,L", [(21, 9), (32, 12)])
 def test_c64_with_vacancies_and_odd_width(rgf, plan, oracle, M, L):
     on = inputs.anderson(M, L, 0.2, 7 * M)
