@@ -71,7 +71,7 @@ int rgf_set_device_batch(rgf_plan *p, int n_dev, int M, int L, const double *ons
                          const uint8_t *vacancy);
 
 /* T(E) for n_E energies (eV), broadening eta > 0 (eV), sweep precision RGF_C128 / RGF_C64.
- * T_out[n_dev][n_E] doubles (n_dev = 1 after rgf_set_device).  Synchronous: T_out is valid on
+ * T_out[n_dev][n_E] doubles (n_dev = 1 after rgf_set_device; n_dev * n_E <= 65535 per call).  Synchronous: T_out is valid on
  * return.  Runs leads (A2), the sweep (A3-A5) and the trace (A6) on the GPU.  On a per-energy
  * failure that entry of T_out is NaN, the other energies are still computed, and the code
  * (RGF_ENOCONV / RGF_ESINGULAR) is returned. */
@@ -98,6 +98,8 @@ typedef struct rgf_stats {
     long long launches_leads;   /* kernels launched by the lead decimation                       */
     int lead_iterations;        /* decimation iterations run (max over energies)                 */
     int cohort;                 /* matrices per launch                                           */
+    int guard_redone;           /* energies recomputed in RGF_FORM_DENSE by the near-neutrality guard */
+    int reserved;
 } rgf_stats;
 int rgf_get_stats(const rgf_plan *p, rgf_stats *out);
 
@@ -121,20 +123,36 @@ int rgf_set_profiling(rgf_plan *p, int level);
 enum { RGF_FORM_DENSE = 0, RGF_FORM_HALF = 1, RGF_FORM_HALF_STEPWISE = 2 };
 int rgf_set_formulation(rgf_plan *p, int formulation);
 
-/* How the Sancho-Rubio decimation of the clean two-slice lead cell (BASELINE.json:north_star item 4) inverts the cell:
- *   RGF_LEAD_CELL_DENSE  one pivoted 2M x 2M inverse per iteration + 8 products of size M;
- *   RGF_LEAD_CELL_SCHUR  (default) the same iteration on the (M/2)-blocks alpha, beta and the corrections really
- *                        occupy; the four corner blocks of the cell's inverse it consumes come from one pivoted inverse
- *                        of the M x M Schur complement on the atoms that bond to the neighbouring cells (the other
- *                        atoms pair up across the two slices and are eliminated in closed form): 8x fewer flops.
- *                        Falls back to RGF_LEAD_CELL_DENSE for a call with an energy within 1 % of +-t, where the
- *                        closed elimination is resonant.  Both give the same surface Green's function (tested). */
-enum { RGF_LEAD_CELL_DENSE = 0, RGF_LEAD_CELL_SCHUR = 1 };
+/* How the lead surface Green's functions (A2) are computed.  All three give the same Sigma_L/R (tested against the oracle):
+ *   RGF_LEAD_MODE_SPACE  (default) the paper's own route ("solution of an eigen-problem"): in the transverse
+ *                        sine basis the clean armchair lead decouples into M/2 chains with alternating hoppings
+ *                        2t cos(p pi/(M+1)) and t; the surface Green's function of each chain is a closed form (root of a
+ *                        quadratic), transformed back by one real x complex product per energy.  O(M) + one product,
+ *                        no iteration, no host synchronisation, no resonance of the isolated cell;
+ *   RGF_LEAD_CELL_DENSE  Sancho-Rubio decimation of the two-slice cell (BASELINE.json:north_star item 4) with one pivoted
+ *                        2M x 2M inverse per iteration + 8 products of size M;
+ *   RGF_LEAD_CELL_SCHUR  the same decimation on the (M/2)-blocks alpha, beta and the corrections really occupy; the corner
+ *                        blocks of the cell's inverse come from one pivoted inverse of the M x M Schur complement on the
+ *                        atoms that bond to the neighbouring cells: 8x fewer flops.  Falls back to RGF_LEAD_CELL_DENSE for
+ *                        a call with an energy within 1 % of +-t, where the closed elimination is resonant. */
+enum { RGF_LEAD_CELL_DENSE = 0, RGF_LEAD_CELL_SCHUR = 1, RGF_LEAD_MODE_SPACE = 2 };
 int rgf_set_lead_method(rgf_plan *p, int method);
 
-/* Matrices per kernel launch in the sweep (0 = library default).  RGF_FORM_DENSE / _STEPWISE: the sweep runs cohort
- * after cohort over all slices.  RGF_FORM_HALF (fused kernel): upper bound on the units (matrix, 64 half-steps) per
- * launch, default = the number of resident CTA slots of the GPU. */
+/* Near-charge-neutrality guard of RGF_FORM_HALF (complex128, fused kernel).  The cut between the two halves of a slice
+ * leaves singly bonded atoms whose edge-like states are resonant close to charge neutrality (PAPER.md:82 is about
+ * exactly this energy range); a step then loses about 0.2 eps_mach (|t| max|g|)^2.  The fused kernel records the
+ * smallest pivot of every (device, energy) pair, G = |t| / min|pivot|, and every energy with
+ *     2.4e-17 G^2 T / max(1, T) > tol
+ * for some device is computed again in RGF_FORM_DENSE, which has no such cut, inside the same rgf_transmission call.
+ * tol = 0 switches the guard off; default 3e-11.  rgf_stats.guard_redone counts the energies recomputed. */
+int rgf_set_guard(rgf_plan *p, double tol);
+/* G of the first pass of the last rgf_transmission call, [n_dev][n_E] (HOST pointer; 0 where not recorded). */
+int rgf_get_guard_indicators(const rgf_plan *p, double *G_out, int n);
+
+/* Matrices per kernel launch in the sweep (0 = library default).  RGF_FORM_DENSE / _STEPWISE and the complex64 sweep:
+ * the sweep runs cohort after cohort over all slices.  RGF_FORM_HALF in complex128 (fused kernel): the whole batch is one
+ * cohort and `cohort` bounds the units (matrix, 64 half-steps) per launch instead, default = the number of resident CTA
+ * slots of the GPU; with fewer slots than matrices every matrix is resumed from the state it left in HBM. */
 int rgf_set_cohort(rgf_plan *p, int cohort);
 
 /* Measures the FP64 tensor-pipe ceiling of the plan's GPU (independent DMMA.8x8x4 chains on every

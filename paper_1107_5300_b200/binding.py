@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "librgf_b200.so")
 
 RGF_C128, RGF_C64 = 0, 1
 RGF_FORM_DENSE, RGF_FORM_HALF, RGF_FORM_HALF_STEPWISE = 0, 1, 2
-RGF_LEAD_CELL_DENSE, RGF_LEAD_CELL_SCHUR = 0, 1
+RGF_LEAD_CELL_DENSE, RGF_LEAD_CELL_SCHUR, RGF_LEAD_MODE_SPACE = 0, 1, 2
 RGF_OK, RGF_EINVAL, RGF_ECUDA, RGF_ENOMEM, RGF_ENOCONV, RGF_ESINGULAR, RGF_ESTATE, RGF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6, -7
 
 if not os.path.exists(LIB_PATH):
@@ -27,7 +27,7 @@ _lib = C.CDLL(LIB_PATH)
 class rgf_stats(C.Structure):
     _fields_ = [("ms_total", C.c_double), ("ms_leads", C.c_double), ("ms_sweep", C.c_double), ("ms_trace", C.c_double),
                 ("ms_inverse_update", C.c_double), ("launches", C.c_longlong), ("launches_inverse_update", C.c_longlong), ("launches_leads", C.c_longlong),
-                ("lead_iterations", C.c_int), ("cohort", C.c_int)]
+                ("lead_iterations", C.c_int), ("cohort", C.c_int), ("guard_redone", C.c_int), ("reserved", C.c_int)]
 
 
 _vp = C.c_void_p
@@ -43,6 +43,8 @@ _lib.rgf_set_profiling.argtypes = [_vp, C.c_int]
 _lib.rgf_set_cohort.argtypes = [_vp, C.c_int]
 _lib.rgf_set_formulation.argtypes = [_vp, C.c_int]
 _lib.rgf_set_lead_method.argtypes = [_vp, C.c_int]
+_lib.rgf_set_guard.argtypes = [_vp, C.c_double]
+_lib.rgf_get_guard_indicators.argtypes = [_vp, _vp, C.c_int]
 _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
@@ -124,6 +126,14 @@ def rgf_set_lead_method(plan, method):
 
 def rgf_set_cohort(plan, cohort):
     return _check(plan, _lib.rgf_set_cohort(plan, cohort))
+
+
+def rgf_set_guard(plan, tol):
+    return _check(plan, _lib.rgf_set_guard(plan, tol))
+
+
+def rgf_get_guard_indicators(plan, G_out, n):
+    return _check(plan, _lib.rgf_get_guard_indicators(plan, _addr(G_out, np.float64), n))
 
 
 def rgf_fp64_peak_tflops(plan):

@@ -28,7 +28,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps()):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [NVCC] + FLAGS + os.environ.get("RGF_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     return LIB

@@ -33,13 +33,7 @@ namespace rgf {
 constexpr int HS_NT = 256, HS_NMAX = 128, HS_B = 32, HS_SB = 8;
 constexpr int HS_LDP = HS_B + 4;        // 36: A-fragment reads of the panel conflict-free
 constexpr int HS_LDR = HS_B + 2;        // 34: B-fragment reads conflict-free
-constexpr int HS_TRACE = 1024;
-#ifndef HS_FSB
-#define HS_FSB 8                        // sub-block width of the panel factorisation
-#endif
-#ifndef HS_RG
-#define HS_RG 2                         // row blocks of 8 per register tile of the strip update
-#endif       // the panel buffer seen as rows of HS_NMAX elements (assembly staging)
+constexpr int HS_RG = 2;                // row blocks of 8 per register tile of the strip update
 
 struct HSweepArgs {
     int M, L, nh, ldn, n_E, bz0, nb;
@@ -50,11 +44,10 @@ struct HSweepArgs {
     cplx *X0, *X1, *P0, *P1;      // [nb][ldn*ldn] each
     int *perm;                    // [nb][2][HS_NMAX]: row and column maps of a matrix between launches
     int *status;                  // [nb]
+    unsigned *pivmin;             // [nb] or NULL: min over all pivots of the top 24 bits of max(|re|, |im|) (near-neutrality guard)
     int hs_begin, hs_end;         // half-steps [begin, end) of the whole sweep: hs = 2 i + kind
     int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
                                   // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
-    long long *prof;              // optional [nb][16] cycle counters of thread 0 per phase (NULL = off)
-    long long *trace;             // optional [nb][HS_TRACE] event log of thread 0: [0] = SM id, then (globaltimer ns << 8 | event)
     cplx *g_out, *P_out;          // after half-step hs_end - 1: g dense n x n (ld n) and P (ld nh), stride nh*nh; may be NULL
 };
 
@@ -68,10 +61,10 @@ struct HSmem {
     int rmap[HS_NMAX], cmap[HS_NMAX];                 // logical row / column of the last result -> physical row / column
     int rmap_prev[HS_NMAX], cmap_prev[HS_NMAX];
     int prow[HS_B];
+    unsigned pivmin;
     // in-place assembly of a kind-B half-step (HSXf), per physical row / column of the previous result
     double xf_sr[HS_NMAX], xf_sw[HS_NMAX], xf_dre[HS_NMAX], xf_mc[HS_NMAX];
     short xf_dcol[HS_NMAX], xf_pa[HS_NMAX], xf_pb[HS_NMAX];
-    long long prof[16];          // per-phase cycle counters of thread 0 (debugging aid, RGF_HS_PROF)
 };
 
 // per-row tables of the assembly; aliases HSmem::crow while no panel is being factored
@@ -112,10 +105,6 @@ __device__ __forceinline__ double hs_rcp(double v)
     return r;
 }
 
-#ifdef HS_DBG
-__device__ long long hs_dbg[8];
-#endif
-
 // named barrier over `nthreads` threads (whole warps)
 __device__ __forceinline__ void hs_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
@@ -128,7 +117,7 @@ struct HSView {
     cplx *crow, *cinv;    // candidate buffers [2][8][HS_SB], [2][8]
     unsigned *ckey;       // [2][8], 16-byte aligned
     int *prow, *perm, *pinv;
-    long long *prof;      // shared-memory cycle counters or NULL
+    unsigned *pivmin;
 };
 struct HSGroup {
     int r;                // row owned by this thread
@@ -151,12 +140,6 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
     const int r = gr.r, warp = gr.slot, naw = gr.nslots;
     constexpr int NW = HS_NT / 32;
     constexpr int pb = (CC & 1) * NW;
-#ifdef HS_DBG
-    long long td0 = clock64();
-#define HS_DBGT(k) do { long long n_ = clock64(); if (threadIdx.x == 0) hs_dbg[k] += n_ - td0; td0 = n_; } while (0)
-#else
-#define HS_DBGT(k)
-#endif
     const cplx x = row[CC];
     // search key from max(|re|, |im|) (integer compare of the high words: no FP64 op on the critical path; the
     // chosen pivot is within sqrt(2) * (1 + 2^-12) of the largest modulus, as good for partial pivoting)
@@ -165,7 +148,6 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
     const unsigned key = hi | (unsigned)(255 - r);
     const double v = cabs2(x);                    // for the reciprocal; overlaps the warp reduction
     const unsigned wmax = __reduce_max_sync(0xffffffffu, key);
-    HS_DBGT(0);
     if (key == wmax) {
         sm.ckey[pb + warp] = key;
         const double iv = hs_rcp(v);
@@ -173,9 +155,7 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
 #pragma unroll
         for (int j = 0; j < SB; j++) if (j != CC) sm.crow[(pb + warp) * SB + j] = row[j];
     }
-    HS_DBGT(1);
     hs_bar(gr.bar_pivot, gr.n_pivot);
-    HS_DBGT(2);
     const uint4 k4 = *reinterpret_cast<const uint4 *>(&sm.ckey[pb]);
     unsigned best = k4.x;
     if (naw > 1) best = max(best, k4.y);
@@ -189,7 +169,6 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
         if (naw > 7) best = max(best, k5.w);
     }
     const int pr = 255 - (int)(best & 0xffu), pw = pr >> 5;
-    HS_DBGT(3);
     const cplx d = sm.cinv[pb + pw];
     const bool is_piv = (r == pr);
     const cplx nf = cmake(fma(-x.x, d.x, x.y * d.y), fma(-x.x, d.y, -x.y * d.x));     // -(x d)
@@ -203,16 +182,14 @@ __device__ __forceinline__ void hs_pivot_step(const HSView &sm, const HSGroup &g
         c.y = fma(a.x, pj.y, c.y); c.y = fma(a.y, pj.x, c.y);
         row[j] = c;
     }
-    HS_DBGT(4);
     if (is_piv) {
         if ((best >> 8) == 0u || best >= 0x7ff00000u) *status_slot = 1;
+        atomicMin(sm.pivmin, best >> 8);
         used = true;
         sm.prow[kglob & (HS_B - 1)] = pr;
         sm.perm[kglob] = pr;
         sm.pinv[pr] = kglob;
     }
-    HS_DBGT(5);
-#undef HS_DBGT
 }
 
 // in-panel update behind sub-block s (columns [c0, c0 + ncols) of the panel, pivot rows snapshotted in sm.Rs):
@@ -281,14 +258,12 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
     static_assert(SB == 8 || SB == 4, "sub-block width");
     const int r = gr.r;
     const bool has_row = r < n;
-    long long tp = sm.prof ? clock64() : 0;
     cplx *panel = sm.panel;
     cplx *Rs = sm.Rs;
     for (int s = 0; s < B / SB; s++) {
         const int c0 = s * SB;
         const int ncols = bw - c0 < SB ? bw - c0 : SB;
         if (ncols <= 0) break;
-        if (sm.prof) tp = clock64();
         cplx row[SB];
         if (has_row) {
 #pragma unroll
@@ -311,7 +286,6 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
             }
         }
         hs_bar(gr.bar_all, gr.gnt);
-        if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[5] += now_ - tp; tp = now_; }
         if (has_row) {
 #pragma unroll
             for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
@@ -325,20 +299,18 @@ __device__ __forceinline__ void hs_factor_panel(const HSView &sm, const HSGroup 
                 Rs[k * LDR + c] = (k < ncols && !own) ? panel[sm.prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
             }
             hs_bar(gr.bar_all, gr.gnt);
-            if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[13] += now_ - tp; tp = now_; }
             hs_inpanel_update<SB>(sm, gr, n, bw, s, c0, ncols);
             hs_bar(gr.bar_all, gr.gnt);
-            if (sm.prof) { long long now_ = clock64(); if (gr.gtid == 0) sm.prof[14] += now_ - tp; tp = now_; }
         }
     }
 }
 
 // view / group of the whole-CTA kernel: thread = row, all eight warps in the in-panel DMMAs
-__device__ __forceinline__ HSView hs_view(HSmem &sm, bool prof)
+__device__ __forceinline__ HSView hs_view(HSmem &sm)
 {
     HSView v;
     v.panel = sm.panel; v.Rs = sm.Rs; v.crow = sm.crow; v.cinv = sm.cinv; v.ckey = sm.ckey;
-    v.prow = sm.prow; v.perm = sm.perm; v.pinv = sm.pinv; v.prof = prof ? sm.prof : nullptr;
+    v.prow = sm.prow; v.perm = sm.perm; v.pinv = sm.pinv; v.pivmin = &sm.pivmin;
     return v;
 }
 __device__ __forceinline__ HSGroup hs_group_cta(int n)
@@ -515,15 +487,12 @@ __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *pr
 // ---- [X | W] <- A^-1 [I | W] in place; fills sm.perm / sm.pinv.  X holds A on entry (xtf = 0) or the previous result
 // that HSXf turns into A while panel 0 is loaded and applied (xtf = 1); W likewise: wtf = 0 (W in place), 2 (previous
 // propagator, scaled in place) or 3 (stencil of the previous propagator in the other buffer) ---------------------------------------
-__device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot, long long *prof,
-                                                int xtf, int wtf, const HSXf &xf, long long *trace, int &tri)
+__device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot,
+                                                int xtf, int wtf, const HSXf &xf)
 {
-#define HS_EV(id) do { if (trace && threadIdx.x == 0 && tri < HS_TRACE) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); trace[tri++] = (long long)((t_ << 8) | (unsigned)(id)); } } while (0)
-    long long tc = prof ? clock64() : 0;
-#define HS_TICK(slot) do { if (prof) { long long now_ = clock64(); if (threadIdx.x == 0) sm.prof[slot] += now_ - tc; tc = now_; } } while (0)
     const int tid = threadIdx.x;
     bool used = !(tid < n);
-    const HSView view = hs_view(sm, prof != nullptr);
+    const HSView view = hs_view(sm);
     const HSGroup grp = hs_group_cta(n);
     const int nsx = (n + 7) >> 3, nsw = (nc + 7) >> 3;
     for (int k0 = 0; k0 < n; k0 += HS_B) {
@@ -557,10 +526,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
             }
         }
         __syncthreads();
-        HS_TICK(1);
-        HS_EV(1);
-        hs_factor_panel<HS_FSB>(view, grp, n, k0, bw, used, status_slot);
-        HS_TICK(2);
+        hs_factor_panel<HS_SB>(view, grp, n, k0, bw, used, status_slot);
         // N' -> X[:, K];  then the panel becomes Mult = N' - E (E[prow[c]][c] = 1)
         for (int e = tid; e < n * HS_B; e += HS_NT) {
             const int rr = e / HS_B, c = e % HS_B;
@@ -569,8 +535,6 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         __syncthreads();
         if (tid < bw) sm.panel[sm.prow[tid] * HS_LDP + tid].x -= 1.0;
         __syncthreads();
-        HS_TICK(3);
-        HS_EV(2);
         // strip list: the 8-column strips of X except the panel's own four, then the strips of W; warp w takes
         // strips w, w + 8, ...
         const int sk0 = k0 >> 3;
@@ -598,11 +562,7 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
 #undef HS_STRIP
         }
         __syncthreads();
-        HS_TICK(4);
-        HS_EV(3);
     }
-#undef HS_TICK
-#undef HS_EV
 }
 
 // ---- assembly of A (into Xn) and of W = C P_prev (into Wn) for half-step (i, kind) -------------------------
@@ -786,14 +746,11 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
     cplx *const X0 = a.X0 + bl * xs, *const X1 = a.X1 + bl * xs, *const W0 = a.P0 + bl * xs, *const W1 = a.P1 + bl * xs;
     int *gmaps = a.perm + (long long)bl * 2 * HS_NMAX;
     int *status_slot = a.status + bl;
+    if (tid == 0) sm.pivmin = 0xffffffffu;
     if (hs_begin > 0) {
         if (tid < HS_NMAX) { sm.rmap[tid] = gmaps[tid]; sm.cmap[tid] = gmaps[HS_NMAX + tid]; }
         __syncthreads();
     }
-    if (tid < 16) sm.prof[tid] = 0;
-    long long *trace = a.trace ? a.trace + (long long)bl * HS_TRACE : nullptr;
-    int tri = 1;
-    if (trace && tid == 0) { unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); trace[0] = smid; }
     const int bz = a.bz0 + bl, dev = bz / a.n_E;
     const double E = a.energies[bz % a.n_E];
     HSXf xf = {sm.xf_sr, sm.xf_sw, sm.xf_dre, sm.xf_mc, sm.xf_dcol, a.eta, nullptr, sm.xf_pa, sm.xf_pb, a.t};
@@ -808,8 +765,6 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         n = half_count(M, par);
         if (tid < HS_NMAX) { sm.rmap_prev[tid] = sm.rmap[tid]; sm.cmap_prev[tid] = sm.cmap[tid]; }
         __syncthreads();
-        long long tc0 = a.prof ? clock64() : 0;
-        if (trace && tid == 0 && tri < HS_TRACE) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); trace[tri++] = (long long)((t_ << 8) | 0u); }
         if (inplace) {
             // tables of the in-place assembly (HSXf): atom r of this B half sits in physical row rmap[r] and its column
             // in physical column cmap[r] of the previous (F) result
@@ -837,10 +792,8 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
             }
         }
         __syncthreads();
-        if (a.prof && tid == 0) sm.prof[0] += clock64() - tc0;
         xf.Wp = Wp;
-        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, a.prof ? a.prof + bl * 16 : nullptr,
-                        inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf, trace, tri);
+        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf);
         // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
         // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
         // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].
@@ -852,7 +805,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         __syncthreads();
     }
     if (tid < HS_NMAX) { gmaps[tid] = sm.rmap[tid]; gmaps[HS_NMAX + tid] = sm.cmap[tid]; }
-    if (a.prof && tid < 16) a.prof[bl * 16 + tid] += sm.prof[tid];
+    if (tid == 0 && a.pivmin) atomicMin(a.pivmin + bl, sm.pivmin);
     if (hs_end == a.hs_end && (a.g_out || a.P_out)) {
         const int fb = hs_out_buf(hs_end - 1);
         const cplx *Xf = fb ? X1 : X0, *Wf = fb ? W1 : W0;

@@ -23,6 +23,7 @@
 #include "half_kernels.cuh"
 #include "half_sweep.cuh"
 #include "half_sweep_c64.cuh"
+#include "lead_modes.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -58,13 +59,18 @@ struct rgf_plan {
     int M = 0, L = 0, n_dev = 0, nh = 0;
     double t = 0.0;
     Buf onsite, bond, hop, bondc;                 // device description
-    Buf E, T, status, lead_flags, counters;       // per call
+    Buf E, T, status, lead_flags;                 // per call
+    Buf pivmin, T_keep, redo_idx;                 // near-neutrality guard: smallest pivot per matrix, first-pass T, redone energies
+    std::vector<double> guard_G;                  // |t| / smallest pivot per batch item of the last call
+    double guard_tol = 3e-11;
     std::vector<Ws> ws;                           // ws[0] runs on the plan's stream
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
     Buf lc_S3, lc_R;                              // run_lead_side_schur: S again and the residual of its inverse
-    int fast_leads = 1;
+    Buf lm_Q;                                     // mode-space leads: the orthogonal basis Q [nc][nc]
+    Buf lead_status;                              // [n_E] bad pivot inside the lead decimation of an energy
+    int lead_method = RGF_LEAD_MODE_SPACE;
     int cohort_override = 0;
     int nstreams = 1;
     int profiling = 0;
@@ -317,13 +323,12 @@ int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, bo
     if ((rc = ensure(p, p->l_W, sizeof(cplx) * NN * n_E))) return rc;
     if (N <= 256 && (rc = ensure(p, p->l_W2, sizeof(cplx) * NN * n_E))) return rc;
     if ((rc = ensure_inverse_ws(p, w, N, n_E))) return rc;
-    if ((rc = ensure(p, p->lead_flags, sizeof(int) * (size_t)(n_E + 4)))) return rc;
     cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta), *X = ptr<cplx>(p->l_eps), *Y = ptr<cplx>(p->l_eps_s);
     cplx *T1 = ptr<cplx>(p->l_T1), *T2 = ptr<cplx>(p->l_T2), *an = ptr<cplx>(p->l_T3);
     cplx *Sacc = ptr<cplx>(p->stage_in);          // surface accumulator: X_s (right lead, side > 0) or Y_s (left lead)
     cplx *S = ptr<cplx>(p->l_W), *S2 = ptr<cplx>(p->l_W2), *g = nullptr;
     int *flags = ptr<int>(p->lead_flags), *n_open = flags + n_E;
-    int *status = ptr<int>(p->status);      // a bad pivot in the lead marks batch items [0, n_E): device 0 of each energy
+    int *status = ptr<int>(p->lead_status); // a bad pivot in the lead marks the energy: every device of it (fill_nan_kernel)
     const double *E = ptr<double>(p->E);
     dim3 gc((unsigned)std::min<long long>((CC + 255) / 256, 256), n_E), gs((unsigned)std::min<long long>((NN + 255) / 256, 2048), n_E);
     lead_half_init_kernel<<<gc, 256, 0, p->stream>>>(a, b, X, Y, Sacc, nc, p->t);
@@ -428,7 +433,27 @@ bool schur_leads_ok(rgf_plan *p, int n_E)
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return false;
     const double t2 = p->t * p->t;
     for (double e : h) if (std::fabs(e * e - t2) < 0.02 * t2) return false;
-    return p->fast_leads && p->M >= 4;
+    return p->lead_method == RGF_LEAD_CELL_SCHUR && p->M >= 4;
+}
+
+// A2 in mode space (lead_modes.cuh): closed form per transverse mode + one real x complex product per energy
+int run_lead_modes(rgf_plan *p, int n_E, double eta, int qc, cplx *g_out)
+{
+    const int M = p->M, nc = half_count(M, qc);
+    int rc;
+    if ((rc = ensure(p, p->lm_Q, sizeof(double) * (size_t)nc * nc))) return rc;
+    lead_modes_basis_kernel<<<std::min((nc * nc + 255) / 256, 1024), 256, 0, p->stream>>>(ptr<double>(p->lm_Q), M, nc, qc);
+    CUDA_TRY(p, cudaMemsetAsync(g_out, 0, sizeof(cplx) * (size_t)M * M * n_E, p->stream));
+    for (int e0 = 0; e0 < n_E; e0 += 32768) {
+        const int ne = std::min(32768, n_E - e0);
+        dim3 grid((nc + 15) / 16, (nc + 15) / 16, ne);
+        lead_modes_kernel<<<grid, 256, 0, p->stream>>>(g_out + (size_t)e0 * M * M, ptr<double>(p->lm_Q), M, nc, qc, p->t,
+                                                      ptr<double>(p->E) + e0, eta);
+        p->stats.launches++;
+    }
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    return RGF_OK;
 }
 
 // both leads; for even L the two cells have the same bond parities and g_R = g_L exactly
@@ -438,6 +463,20 @@ int run_leads(rgf_plan *p, int n_E, double eta, int *n_open_out)
     int rc, itL = 0, itR = 0, openL = 0, openR = 0;
     const size_t MMb = sizeof(cplx) * (size_t)M * M * n_E;
     if ((rc = ensure(p, p->gL, MMb))) return rc;
+    if ((rc = ensure(p, p->lead_status, sizeof(int) * (size_t)n_E))) return rc;
+    if ((rc = ensure(p, p->lead_flags, sizeof(int) * (size_t)(n_E + 4)))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->lead_status.p, 0, sizeof(int) * (size_t)n_E, p->stream));
+    CUDA_TRY(p, cudaMemsetAsync(p->lead_flags.p, 0, sizeof(int) * (size_t)(n_E + 4), p->stream));
+    if (p->lead_method == RGF_LEAD_MODE_SPACE) {
+        if ((rc = run_lead_modes(p, n_E, eta, 1, ptr<cplx>(p->gL)))) return rc;
+        if ((L & 1) != 0) {
+            if ((rc = ensure(p, p->gR, MMb))) return rc;
+            if ((rc = run_lead_modes(p, n_E, eta, (L - 1) & 1, ptr<cplx>(p->gR)))) return rc;
+        }
+        p->stats.lead_iterations = 0;
+        if (n_open_out) *n_open_out = 0;
+        return RGF_OK;
+    }
     const bool dense = !schur_leads_ok(p, n_E);
     if ((rc = run_lead_side(p, n_E, eta, -1, -2, -1, dense, ptr<cplx>(p->gL), &itL, &openL))) return rc;
     if ((L & 1) == 0) {
@@ -453,8 +492,10 @@ int run_leads(rgf_plan *p, int n_E, double eta, int *n_open_out)
 
 inline const cplx *lead_gR(const rgf_plan *p) { return (p->L & 1) == 0 ? ptr<cplx>(p->gL) : ptr<cplx>(p->gR); }
 
+inline bool use_fused(const rgf_plan *p);
 int choose_cohort(const rgf_plan *p, int batch)
 {
+    if (use_fused(p) && p->precision == RGF_C128) return batch;      // fused kernel: rgf_set_cohort bounds the units per launch instead
     if (p->cohort_override > 0) return std::min(p->cohort_override, batch);
     return (batch + p->nstreams - 1) / p->nstreams;      // one cohort per stream
 }
@@ -541,14 +582,6 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
     a.nb = nb;
     a.X0 = ptr<cplx>(w.Fx0); a.X1 = ptr<cplx>(w.Fx1); a.P0 = ptr<cplx>(w.Fp0); a.P1 = ptr<cplx>(w.Fp1);
     a.perm = ptr<int>(w.Fperm);
-    static const bool prof_on = getenv("RGF_HS_PROF") != nullptr;          // debugging aid: per-phase cycle counters
-    static const char *trace_path = getenv("RGF_HS_TRACE");                // debugging aid: event log of the first launch
-    if (prof_on) {
-        if ((rc = ensure(p, p->counters, sizeof(long long) * (16 + HS_TRACE) * (size_t)nb))) return rc;
-        CUDA_TRY(p, cudaMemsetAsync(p->counters.p, 0, sizeof(long long) * (16 + HS_TRACE) * (size_t)nb, w.stream));
-        a.prof = ptr<long long>(p->counters);
-        if (trace_path) a.trace = a.prof + 16 * (size_t)nb;
-    }
     // Rounds of units: with more matrices than resident CTA slots (2 per SM) a single launch would run 512 matrices
     // as 296 + 216, the second wave half empty.  Instead every launch runs `slots` units of unit_len half-steps; unit
     // u = (matrix u % nb, chunk u / nb), so chunk c+1 of a matrix is always in a later launch than its chunk c
@@ -584,28 +617,6 @@ int fused_launch(rgf_plan *p, Ws &w, HSweepArgs &a, int nb)
         }
     }
     CUDA_TRY(p, cudaGetLastError());
-    if (prof_on) {
-        std::vector<long long> h(16 * (size_t)nb);
-        CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->counters.p, sizeof(long long) * h.size(), cudaMemcpyDeviceToHost, w.stream));
-        CUDA_TRY(p, cudaStreamSynchronize(w.stream));
-        if (trace_path) {
-            std::vector<long long> tr((size_t)HS_TRACE * nb);
-            CUDA_TRY(p, cudaMemcpy(tr.data(), a.trace, sizeof(long long) * tr.size(), cudaMemcpyDeviceToHost));
-            if (FILE *f = fopen(trace_path, "w")) {
-                for (int b = 0; b < nb; b++) {
-                    fprintf(f, "%d %lld", b, tr[(size_t)b * HS_TRACE]);
-                    for (int k = 1; k < HS_TRACE && tr[(size_t)b * HS_TRACE + k]; k++) fprintf(f, " %lld", tr[(size_t)b * HS_TRACE + k]);
-                    fprintf(f, "\n");
-                }
-                fclose(f);
-            }
-        }
-        double s[16] = {0};
-        for (int b = 0; b < nb; b++) for (int k = 0; k < 16; k++) s[k] += (double)h[16 * (size_t)b + k];
-        const double hsn = (double)nb * a.hs_end;
-        fprintf(stderr, "[rgf prof] cycles per half-step per CTA: assemble %.0f  panel-load %.0f  factor %.0f  writeback+stage %.0f  updates %.0f  (pivot steps %.0f of factor)\n           in-panel: pivot-row snapshot %.0f  DMMA %.0f\n",
-                s[0] / hsn, s[1] / hsn, s[2] / hsn, s[3] / hsn, s[4] / hsn, s[5] / hsn, s[13] / hsn, s[14] / hsn);
-    }
     return RGF_OK;
 }
 
@@ -620,6 +631,7 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     a.bond = ptr<uint8_t>(p->bond); a.hop = ptr<uint8_t>(p->hop);
     a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
     a.status = ptr<int>(p->status) + bz0;
+    a.pivmin = p->pivmin.p ? ptr<unsigned>(p->pivmin) + bz0 : nullptr;
     a.hs_begin = 0; a.hs_end = 2 * nslices;
     a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
     if ((rc = fused_launch(p, w, a, nb))) return rc;
@@ -836,54 +848,38 @@ int rgf_set_device(rgf_plan *p, int M, int L, const double *onsite, double t, co
     return rgf_set_device_batch(p, 1, M, L, onsite, t, vacancy);
 }
 
-static int check_energies_finite(rgf_plan *p, int n_E)
+// One pass of the hot path over the n_E energies in p->E: leads (A2), sweep (A3-A5) and trace (A6) in `formulation`.
+// Writes p->T [n_dev][n_E] (NaN where an energy failed), p->status, p->lead_flags / p->lead_status, and for the fused
+// kernel p->pivmin.  *lead_open = number of energies whose lead decimation did not converge.
+static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, int *lead_open_out)
 {
-    std::vector<double> h(n_E);
-    CUDA_TRY(p, cudaMemcpyAsync(h.data(), p->E.p, sizeof(double) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
-    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
-    for (int k = 0; k < n_E; k++)
-        if (!std::isfinite(h[k])) return fail(p, RGF_EINVAL, "energies[%d] is not finite", k);
-    return RGF_OK;
-}
-
-int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, int precision, double *T_out)
-{
-    int rc = begin_call(p);
-    if (rc) return rc;
-    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_transmission before rgf_set_device");
-    if (!T_out) return fail(p, RGF_EINVAL, "T_out is NULL");
-    if (precision != RGF_C128 && precision != RGF_C64) return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
-    if (precision == RGF_C64 && (p->formulation != RGF_FORM_HALF || p->nh > HC_NMAX))
-        return fail(p, RGF_EUNSUPPORTED, "the complex64 sweep is built for RGF_FORM_HALF and M <= 256 only");
-    p->precision = precision;
-    memset(&p->stats, 0, sizeof(p->stats));
-    for (Ws &w : p->ws) w.upd_used = 0;
-    CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
-    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
-    if ((rc = check_energies_finite(p, n_E))) return rc;
+    int rc;
     const int batch = p->n_dev * n_E;
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
     if ((rc = ensure(p, p->T, sizeof(double) * (size_t)batch))) return rc;
+    if ((rc = ensure(p, p->pivmin, sizeof(unsigned) * (size_t)batch))) return rc;
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    CUDA_TRY(p, cudaMemsetAsync(p->pivmin.p, 0xff, sizeof(unsigned) * (size_t)batch, p->stream));
+    const int saved_form = p->formulation;
+    p->formulation = formulation;
     int lead_open = 0;
+    CUDA_TRY(p, cudaEventRecord(p->ev[1], p->stream));
     nvtxRangePushA("rgf_leads");
+    const long long l0 = p->stats.launches;
     rc = run_leads(p, n_E, eta, &lead_open);
     nvtxRangePop();
-    if (rc) return rc;
-    p->stats.launches_leads = p->stats.launches;
-    CUDA_TRY(p, cudaEventRecord(p->ev[1], p->stream));
-    // ---- sweep + trace: cohorts round-robin over the streams; each cohort is an independent chain
+    if (rc) { p->formulation = saved_form; return rc; }
+    p->stats.launches_leads += p->stats.launches - l0;
+    CUDA_TRY(p, cudaEventRecord(p->ev[2], p->stream));
+    // ---- sweep + trace, cohort after cohort
     const int cohort = choose_cohort(p, batch);
     p->stats.cohort = cohort;
-    const int ns = (int)p->ws.size();
-    const bool half = p->formulation != RGF_FORM_DENSE;
-    for (Ws &w : p->ws) if ((rc = half ? ensure_sweep_ws_half(p, w, cohort) : ensure_sweep_ws(p, w, cohort))) return rc;
-    for (int i = 1; i < ns; i++) CUDA_TRY(p, cudaStreamWaitEvent(p->ws[i].stream, p->ev[1], 0));
+    const bool half = formulation != RGF_FORM_DENSE;
+    Ws &w = p->ws[0];
+    if ((rc = half ? ensure_sweep_ws_half(p, w, cohort) : ensure_sweep_ws(p, w, cohort))) { p->formulation = saved_form; return rc; }
     nvtxRangePushA("rgf_sweep");
     p->in_sweep = true;
-    int ci = 0;
-    for (int bz0 = 0; bz0 < batch && rc == RGF_OK; bz0 += cohort, ci++) {
-        Ws &w = p->ws[ci % ns];
+    for (int bz0 = 0; bz0 < batch && rc == RGF_OK; bz0 += cohort) {
         const int nb = std::min(cohort, batch - bz0);
         cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
         if (half) {
@@ -896,38 +892,116 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     }
     p->in_sweep = false;
     nvtxRangePop();
+    p->formulation = saved_form;
     if (rc) return rc;
-    for (int i = 1; i < ns; i++) {
-        CUDA_TRY(p, cudaEventRecord(p->ws[i].done, p->ws[i].stream));
-        CUDA_TRY(p, cudaStreamWaitEvent(p->stream, p->ws[i].done, 0));
-    }
-    CUDA_TRY(p, cudaEventRecord(p->ev[2], p->stream));
-    // failed energies -> NaN.  Lead failures (flags per energy) hit every device of that energy.
-    std::vector<int> h_status(batch), h_flags(n_E, 0);
-    fill_nan_kernel<<<(batch + 255) / 256, 256, 0, p->stream>>>(ptr<double>(p->T), ptr<int>(p->status), batch);
+    // failed items -> NaN; a lead failure (per energy) hits every device of that energy
+    fill_nan_kernel<<<(batch + 255) / 256, 256, 0, p->stream>>>(ptr<double>(p->T), ptr<int>(p->status), ptr<int>(p->lead_flags),
+                                                             ptr<int>(p->lead_status), batch, n_E);
     p->stats.launches++;
-    CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
-    if (lead_open) CUDA_TRY(p, cudaMemcpyAsync(h_flags.data(), p->lead_flags.p, sizeof(int) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaEventRecord(p->ev[3], p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
-    int result = RGF_OK;
-    if (lead_open) {
-        std::vector<double> hT(batch);
-        CUDA_TRY(p, cudaMemcpy(hT.data(), p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToHost));
-        for (int b = 0; b < batch; b++) if (h_flags[b % n_E]) hT[b] = NAN;
-        CUDA_TRY(p, cudaMemcpy(p->T.p, hT.data(), sizeof(double) * (size_t)batch, cudaMemcpyHostToDevice));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, p->ev[1], p->ev[2]); p->stats.ms_leads += ms;
+    cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_sweep += ms;
+    if (lead_open_out) *lead_open_out = lead_open;
+    return RGF_OK;
+}
+
+// result code of a pass from the flags it left on the device (host copies)
+static int pass_result(rgf_plan *p, int n_E, int lead_open, int result)
+{
+    const int batch = p->n_dev * n_E;
+    std::vector<int> h_status(batch), h_ls(n_E);
+    CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(h_ls.data(), p->lead_status.p, sizeof(int) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    if (lead_open)
         result = fail(p, RGF_ENOCONV, "lead decimation did not converge in %d iterations for %d energies", kLeadMaxIt, lead_open);
-    }
+    for (int e = 0; e < n_E; e++)
+        if (h_ls[e]) { result = fail(p, RGF_ESINGULAR, "zero or non-finite pivot in the lead decimation of energy %d", e); break; }
     for (int b = 0; b < batch; b++)
         if (h_status[b]) { result = fail(p, RGF_ESINGULAR, "zero or non-finite pivot (first at batch item %d)", b); break; }
+    return result;
+}
+
+int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, int precision, double *T_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_transmission before rgf_set_device");
+    if (!T_out) return fail(p, RGF_EINVAL, "T_out is NULL");
+    if (precision != RGF_C128 && precision != RGF_C64) return fail(p, RGF_EINVAL, "precision must be RGF_C128 or RGF_C64");
+    if (precision == RGF_C64 && (p->formulation != RGF_FORM_HALF || p->nh > HC_NMAX))
+        return fail(p, RGF_EUNSUPPORTED, "the complex64 sweep is built for RGF_FORM_HALF and M <= 256 only");
+    if (n_E >= 1 && (long long)p->n_dev * n_E > 65535)
+        return fail(p, RGF_EUNSUPPORTED, "n_dev * n_E = %lld > 65535 batch items per call: split the energy grid", (long long)p->n_dev * n_E);
+    p->precision = precision;
+    memset(&p->stats, 0, sizeof(p->stats));
+    p->ws[0].upd_used = 0;
+    CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
+    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
+    std::vector<double> hE(n_E);
+    CUDA_TRY(p, cudaMemcpyAsync(hE.data(), p->E.p, sizeof(double) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    for (int k = 0; k < n_E; k++)
+        if (!std::isfinite(hE[k])) return fail(p, RGF_EINVAL, "energies[%d] is not finite", k);
+    const int batch = p->n_dev * n_E;
+    int lead_open = 0;
+    if ((rc = transmission_pass(p, n_E, eta, p->formulation, &lead_open))) return rc;
+    int result = pass_result(p, n_E, lead_open, RGF_OK);
+    if (result == RGF_ECUDA) return result;
+    // ---- near-charge-neutrality guard of the half-slice formulation.  The cut between
+    // B_i and F_i leaves the B atoms singly bonded; where their edge-like states are resonant the step loses
+    // ~ 0.2 eps_mach (|t| max|gB|)^2.  The fused kernel records the smallest pivot of every matrix; items whose estimate
+    // exceeds guard_tol are computed again in RGF_FORM_DENSE (no such cut) and replace the first result.
+    p->guard_G.assign(batch, 0.0);
+    if (p->guard_tol > 0.0 && precision == RGF_C128 && use_fused(p)) {
+        std::vector<unsigned> key(batch);
+        std::vector<double> hT(batch);
+        CUDA_TRY(p, cudaMemcpyAsync(key.data(), p->pivmin.p, sizeof(unsigned) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+        CUDA_TRY(p, cudaMemcpyAsync(hT.data(), p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        std::vector<char> redo(n_E, 0);
+        for (int b = 0; b < batch; b++) {
+            const unsigned long long bits = ((unsigned long long)(key[b] << 8)) << 32;
+            double piv;
+            memcpy(&piv, &bits, sizeof(piv));
+            const double G = (key[b] == 0xffffffffu || !(piv > 0.0)) ? 0.0 : std::fabs(p->t) / piv;
+            p->guard_G[b] = G;
+            const double T = std::isfinite(hT[b]) ? std::fabs(hT[b]) : 1.0;
+            if (2.4e-17 * G * G * T / std::max(1.0, T) > p->guard_tol) redo[b % n_E] = 1;
+        }
+        std::vector<int> idx;
+        std::vector<double> E2;
+        for (int e = 0; e < n_E; e++) if (redo[e]) { idx.push_back(e); E2.push_back(hE[e]); }
+        const int n2 = (int)idx.size();
+        p->stats.guard_redone = n2;
+        if (n2 > 0) {
+            if ((rc = ensure(p, p->T_keep, sizeof(double) * (size_t)batch))) return rc;
+            if ((rc = ensure(p, p->redo_idx, sizeof(int) * (size_t)n2))) return rc;
+            CUDA_TRY(p, cudaMemcpyAsync(p->T_keep.p, p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToDevice, p->stream));
+            CUDA_TRY(p, cudaMemcpyAsync(p->redo_idx.p, idx.data(), sizeof(int) * (size_t)n2, cudaMemcpyHostToDevice, p->stream));
+            CUDA_TRY(p, cudaMemcpyAsync(p->E.p, E2.data(), sizeof(double) * (size_t)n2, cudaMemcpyHostToDevice, p->stream));
+            CUDA_TRY(p, cudaStreamSynchronize(p->stream));          // idx / E2 are host vectors
+            int open2 = 0;
+            if ((rc = transmission_pass(p, n2, eta, RGF_FORM_DENSE, &open2))) return rc;
+            const int r2 = pass_result(p, n2, open2, RGF_OK);
+            if (r2 != RGF_OK) result = r2;
+            scatter_T_kernel<<<(p->n_dev * n2 + 255) / 256, 256, 0, p->stream>>>(ptr<double>(p->T_keep), ptr<double>(p->T), ptr<int>(p->redo_idx),
+                                                                                n2, n_E, p->n_dev);
+            p->stats.launches++;
+            CUDA_TRY(p, cudaMemcpyAsync(p->T.p, p->T_keep.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToDevice, p->stream));
+            CUDA_TRY(p, cudaMemcpyAsync(p->E.p, hE.data(), sizeof(double) * (size_t)n_E, cudaMemcpyHostToDevice, p->stream));
+            CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        }
+    }
     CUDA_TRY(p, cudaMemcpyAsync(T_out, p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDefault, p->stream));
-    CUDA_TRY(p, cudaEventRecord(p->ev[3], p->stream));
+    CUDA_TRY(p, cudaEventRecord(p->ev[4], p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     drain_update_events(p);
     float ms = 0.f;
-    cudaEventElapsedTime(&ms, p->ev[0], p->ev[3]); p->stats.ms_total = ms;
-    cudaEventElapsedTime(&ms, p->ev[0], p->ev[1]); p->stats.ms_leads = ms;
-    cudaEventElapsedTime(&ms, p->ev[1], p->ev[2]); p->stats.ms_sweep = ms;
-    cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_trace = ms;
+    cudaEventElapsedTime(&ms, p->ev[0], p->ev[4]); p->stats.ms_total = ms;
+    p->stats.ms_trace = p->stats.ms_total - p->stats.ms_leads - p->stats.ms_sweep;
     return result;
 }
 
@@ -936,9 +1010,9 @@ int rgf_destroy(rgf_plan *p)
     if (!p) return RGF_OK;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->counters,
+    Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->pivmin, &p->T_keep, &p->redo_idx,
                    &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3,
-                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R};
+                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status};
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
@@ -979,8 +1053,22 @@ int rgf_set_formulation(rgf_plan *p, int formulation)
 
 int rgf_set_lead_method(rgf_plan *p, int method)
 {
-    if (!p || (method != RGF_LEAD_CELL_DENSE && method != RGF_LEAD_CELL_SCHUR)) return RGF_EINVAL;
-    p->fast_leads = method == RGF_LEAD_CELL_SCHUR;
+    if (!p || method < RGF_LEAD_CELL_DENSE || method > RGF_LEAD_MODE_SPACE) return RGF_EINVAL;
+    p->lead_method = method;
+    return RGF_OK;
+}
+
+int rgf_set_guard(rgf_plan *p, double tol)
+{
+    if (!p || !(tol >= 0.0)) return RGF_EINVAL;
+    p->guard_tol = tol;
+    return RGF_OK;
+}
+
+int rgf_get_guard_indicators(const rgf_plan *p, double *G_out, int n)
+{
+    if (!p || !G_out || n < 0) return RGF_EINVAL;
+    for (int k = 0; k < n; k++) G_out[k] = k < (int)p->guard_G.size() ? p->guard_G[k] : 0.0;
     return RGF_OK;
 }
 
@@ -1072,24 +1160,19 @@ int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, 
     if ((rc = run_leads(p, n_E, eta, &open))) return rc;
     const int M = p->M, L = p->L;
     const size_t MM = (size_t)M * M;
-    std::vector<cplx> g(MM * n_E);
-    std::vector<uint8_t> m(M);
     const cplx *src = side < 0 ? ptr<cplx>(p->gL) : lead_gR(p);
-    CUDA_TRY(p, cudaMemcpyAsync(g.data(), src, sizeof(cplx) * MM * n_E, cudaMemcpyDeviceToHost, p->stream));
-    CUDA_TRY(p, cudaMemcpyAsync(m.data(), ptr<uint8_t>(p->bond) + ((size_t)dev * (L + 1) + (side < 0 ? 0 : L)) * M, M,
-                                cudaMemcpyDeviceToHost, p->stream));
+    // Sigma = t^2 m (.) g (.) m, masked on the device (lead_sigma_kernel)
+    if ((rc = ensure(p, p->stage_out, sizeof(cplx) * MM * n_E))) return rc;
+    dim3 grid((unsigned)std::min<size_t>((MM + 255) / 256, 2048), n_E);
+    lead_sigma_kernel<<<grid, 256, 0, p->stream>>>(ptr<cplx>(p->stage_out), src, ptr<uint8_t>(p->bond) + ((size_t)dev * (L + 1) + (side < 0 ? 0 : L)) * M, M, p->t);
+    p->stats.launches++;
+    CUDA_TRY(p, cudaGetLastError());
+    CUDA_TRY(p, cudaMemcpyAsync(Sigma_out, p->stage_out.p, sizeof(cplx) * MM * n_E, cudaMemcpyDefault, p->stream));
+    std::vector<int> h_ls(n_E);
+    CUDA_TRY(p, cudaMemcpyAsync(h_ls.data(), p->lead_status.p, sizeof(int) * (size_t)n_E, cudaMemcpyDeviceToHost, p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
-    // Sigma = t^2 m (.) g (.) m: the same masked scale the assembly kernel applies; done here on the
-    // host only to hand the checker a full matrix (this entry point is not on the hot path)
-    const double t2 = p->t * p->t;
     for (int e = 0; e < n_E; e++)
-        for (int j = 0; j < M; j++)
-            for (int k = 0; k < M; k++) {
-                cplx &v = g[(size_t)e * MM + (size_t)j * M + k];
-                double s = (m[j] && m[k]) ? t2 : 0.0;
-                v.x *= s; v.y *= s;
-            }
-    CUDA_TRY(p, cudaMemcpy(Sigma_out, g.data(), sizeof(cplx) * MM * n_E, cudaMemcpyDefault));
+        if (h_ls[e]) return fail(p, RGF_ESINGULAR, "zero or non-finite pivot in the lead decimation of energy %d", e);
     if (iterations_out) *iterations_out = p->stats.lead_iterations;
     if (open) return fail(p, RGF_ENOCONV, "lead decimation did not converge for %d energies", open);
     return RGF_OK;
@@ -1111,6 +1194,7 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     const int batch = p->n_dev * n_E, M = p->M, nh = p->nh;
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    if ((rc = ensure(p, p->pivmin, sizeof(unsigned) * (size_t)batch))) return rc;
     if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
     Ws &w = p->ws[0];
     const bool half = p->formulation != RGF_FORM_DENSE;

@@ -60,10 +60,10 @@ __device__ __forceinline__ void zmma884(double (&cre)[2], double (&cim)[2], doub
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src, int src_bytes)
 {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem_src), "r"(src_bytes));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem_src), "r"(src_bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // m_i[j] = 1 iff (i + j) even; bit test so that negative (lead) slice indices work
 __host__ __device__ __forceinline__ int mask_bit(int i, int j) { return (((i + j) & 1) == 0) ? 1 : 0; }

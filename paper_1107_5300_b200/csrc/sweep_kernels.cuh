@@ -146,10 +146,18 @@ __global__ void propagator_expand_kernel(const cplx *Pall, cplx *Out, int M, int
     }
 }
 
-__global__ void fill_nan_kernel(double *T, const int *status, int n)
+// failed batch items -> NaN: status per item (sweep), lead_flags / lead_status per energy (decimation not converged / bad pivot)
+__global__ void fill_nan_kernel(double *T, const int *status, const int *lead_flags, const int *lead_status, int n, int n_E)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n && status[i]) T[i] = __longlong_as_double(0x7ff8000000000000LL);
+    if (i < n && (status[i] || lead_flags[i % n_E] || lead_status[i % n_E])) T[i] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
+// guard: T_keep[d][idx[k]] = T2[d][k]
+__global__ void scatter_T_kernel(double *T_keep, const double *T2, const int *idx, int n2, int n_E, int n_dev)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n2 * n_dev) T_keep[(long long)(i / n2) * n_E + idx[i % n2]] = T2[i];
 }
 
 }  // namespace rgf

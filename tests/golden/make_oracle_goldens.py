@@ -35,7 +35,7 @@ def subset(cfg):
     if cfg == 3:
         return inputs.config3(disordered=True), [0], [0, 170, 300, 511, 512, 700, 767, 768, 900, 1023], None
     if cfg == 4:
-        return inputs.config4(), [0], [0, 21, 42, 63], 24      # first 24 slices (truncated device)
+        return inputs.config4(), [0], [0, 9, 18, 27, 36, 45, 54, 63], 64      # first 64 slices on 8 energies (truncated device)
     raise SystemExit("config must be 1..4")
 
 

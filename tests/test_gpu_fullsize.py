@@ -85,18 +85,89 @@ def test_config3_clean_c128_closed_form(plan):
 
 
 def test_config4_wide_ribbon_truncated(plan):
-    """configs[4] (M = 1024, edge vacancies): the first 24 slices of the same arrays, leads attached at
-    slice 24 (the naive oracle needs hours per energy at full length), 4 energies."""
-    path = os.path.join(GOLDEN, "config4_oracle.txt")
-    if not os.path.exists(path):
-        pytest.skip("tests/golden/config4_oracle.txt not generated yet")
+    """configs[4] (M = 1024, edge vacancies): the first 64 slices of the same arrays, leads attached at slice 64, on 8
+    energies (the naive oracle needs hours per energy at full length), element = each energy."""
     dev, eidx, E, T_or = golden(4)
-    w = inputs.truncate(inputs.config4(), 24, eidx)
+    assert len(eidx) >= 8
+    w = inputs.truncate(inputs.config4(), 64, eidx)
     assert np.array_equal(w.energies, E)
     plan.set_device(w.onsite, w.t, w.vacancy)
     T = plan.transmission(w.energies, w.eta)[0]
     err = np.abs(T - T_or) / np.maximum(1.0, np.abs(T_or))
     assert np.all(err <= 1e-9), (err.max(), T, T_or)
+
+
+def lapack_referee_T(w, E):
+    """Untimed LAPACK referee: the recursion of north_star written with torch-CPU inv / matmul (MKL), full M x M
+    slices, batched over the energies E; leads by Sancho-Rubio in the M x M block form.  Test code only: it shares nothing
+    with the CUDA path and is not the oracle (it is a library, so it referees where the naive oracle cannot reach)."""
+    import torch
+    M, L, t, eta = w.M, w.L, w.t, w.eta
+    on = torch.from_numpy(w.onsite[0])
+    vac = torch.from_numpy(w.vacancy[0].astype(bool)) if w.vacancy is not None else torch.zeros((L, M), dtype=torch.bool)
+    nE = len(E)
+    z = torch.tensor(E, dtype=torch.complex128) + 1j * eta
+    eye = torch.eye(M, dtype=torch.complex128)
+    j = torch.arange(M)
+
+    def mask(i):
+        return ((i + j) % 2 == 0).to(torch.float64)
+
+    def H(i):            # slice Hamiltonian; i = None: clean lead slice
+        h = torch.zeros((M, M), dtype=torch.complex128)
+        alive = torch.ones(M - 1) if i is None else (~vac[i, :-1] & ~vac[i, 1:]).to(torch.float64)
+        h[j[:-1], j[:-1] + 1] = t * alive.to(torch.complex128)
+        h[j[:-1] + 1, j[:-1]] = t * alive.to(torch.complex128)
+        if i is not None:
+            h[j, j] = on[i].to(torch.complex128)
+        return h
+
+    def lead(pa, pb):    # surface Green's function of the lead cell (pa, pb): eliminate the second slice, decimate M x M blocks
+        va, vb = t * mask(pa), t * mask(pb)
+        G1 = torch.linalg.inv(z[:, None, None] * eye - H(None))
+        eps_s = H(None) + va[:, None] * G1 * va[None, :]
+        eps = eps_s + vb[:, None] * G1 * vb[None, :]
+        al = va[:, None] * G1 * vb[None, :]
+        be = al.transpose(1, 2).clone()
+        for _ in range(64):
+            if max(al.abs().max(), be.abs().max()) < 1e-14:
+                break
+            g = torch.linalg.inv(z[:, None, None] * eye - eps)
+            agb, bga = al @ g @ be, be @ g @ al
+            eps, eps_s = eps + agb + bga, eps_s + agb
+            al, be = al @ g @ al, be @ g @ be
+        return torch.linalg.inv(z[:, None, None] * eye - eps_s)
+
+    gL = lead(-2, -1)
+    gR = gL if L % 2 == 0 else lead(L, L + 1)
+    mL = mask(-1) * (~vac[0]).to(torch.float64)
+    mR = mask(L - 1) * (~vac[L - 1]).to(torch.float64)
+    SigL = (t * mL)[:, None] * gL * (t * mL)[None, :]
+    SigR = (t * mR)[:, None] * gR * (t * mR)[None, :]
+    g = P = None
+    for i in range(L):
+        A = z[:, None, None] * eye - H(i)
+        if i == 0:
+            A = A - SigL
+        else:
+            m = t * mask(i - 1) * (~vac[i - 1]).to(torch.float64) * (~vac[i]).to(torch.float64)
+            A = A - m[:, None] * g * m[None, :]
+        if i == L - 1:
+            A = A - SigR
+        g = torch.linalg.inv(A)
+        P = g[:, :, 1::2].clone() if i == 0 else (g * m[None, :]) @ P      # columns on which Gamma_L lives (odd j)
+    GamL = (1j * (SigL - SigL.conj().transpose(1, 2)))[:, 1::2, 1::2]
+    GamR = 1j * (SigR - SigR.conj().transpose(1, 2))
+    Y = P.conj().transpose(1, 2) @ GamR @ P
+    return torch.einsum("eab,eba->e", GamL, Y).real.numpy()
+
+
+def test_lapack_referee_agrees_with_oracle(oracle):
+    """The referee itself, pinned to the oracle where the oracle is quick (vacancies, odd L, disorder)."""
+    w = inputs.truncate(inputs.config4(M=32, L=21, n_E=6), 21)
+    T_ref = lapack_referee_T(w, w.energies)
+    T_or = oracle.transmission_batch(w.onsite[0], w.vacancy[0], w.t, w.energies, w.eta)
+    assert np.all(np.abs(T_ref - T_or) <= 1e-10 * np.maximum(1.0, T_or)), np.abs(T_ref - T_or)
 
 
 @pytest.mark.parametrize("disordered", [False, True], ids=["clean", "disordered"])
@@ -115,22 +186,15 @@ def test_config3_c64_vs_c128(plan, disordered):
         assert outside.sum() >= 400
     assert np.all(np.isfinite(T64[outside]))       # single precision may overflow only close to charge neutrality (reported)
     d = np.abs(np.where(np.isfinite(T64), T64, 0.0) - T128)
-    if disordered:
-        assert d[outside].max() <= 1e-3, (d[outside].max(), w.energies[outside][np.argmax(d[outside])])
-    else:
-        # Known deviation: with all N_ch <= 34 channels fully open the single-precision noise of
-        # the 4000 half-steps is ~1.7e-5 T (median), so the absolute bound 1e-3 is exceeded where T > 20: measured max
-        # 1.6e-3.  Asserted here: 90 % of the energies within 1e-3, all within 5e-5 T + 1e-3.
-        assert np.quantile(d[outside], 0.90) <= 1e-3, np.quantile(d[outside], 0.90)
-        assert np.all(d[outside] <= 1e-3 + 5e-5 * T128[outside]), (d[outside] / T128[outside]).max()
+    assert d[outside].max() <= 1e-3, (d[outside].max(), w.energies[outside][np.argmax(d[outside])])      # north_star, literally
     assert d.max() > 1e-9          # a different precision really ran
 
 
-def test_config4_wide_ribbon_full_length_properties(plan):
-    """configs[4] at full size (M = 1024, L = 2000, 64 energies, edge vacancies): no oracle value exists at this length
-    (hours per energy), so the properties that hold at any size are checked: finite, 0 <= T <= open lead channels,
-    and the same T from the dense formulation on a sub-sample of energies."""
-    from paper_1107_5300_b200 import binding as rgf
+def test_config4_wide_ribbon_full_length(plan):
+    """configs[4] at full size (M = 1024, L = 2000, 64 energies, edge vacancies) in the launch configuration bench-style
+    runs use.  No oracle value exists at this length (hours per energy with the naive LU), so: the properties that hold at
+    any size on all 64 energies, and the LAPACK referee (lapack_referee_T, untimed, a few minutes of host time) at full
+    length on 2 energies."""
     w = inputs.config4()
     plan.set_device(w.onsite, w.t, w.vacancy)
     T = plan.transmission(w.energies, w.eta)
@@ -139,7 +203,6 @@ def test_config4_wide_ribbon_full_length_properties(plan):
     assert np.all(T >= -1e-9) and np.all(T[0] <= nch + 1e-8), (T.min(), (T[0] - nch).max())
     st = plan.stats()
     print("configs[4] full length: %.1f s (leads %.1f s), %d launches" % (st["ms_total"] / 1e3, st["ms_leads"] / 1e3, st["launches"]))
-    sub = np.array([3, 31, 60])
-    rgf.rgf_set_formulation(plan.handle, rgf.RGF_FORM_DENSE)
-    Td = plan.transmission(w.energies[sub], w.eta)[0]
-    assert np.all(np.abs(Td - T[0, sub]) <= 1e-9 * np.maximum(1.0, Td)), np.abs(Td - T[0, sub])
+    sub = np.array([5, 58])
+    T_ref = lapack_referee_T(w, w.energies[sub])
+    assert np.all(np.abs(T_ref - T[0, sub]) <= 1e-9 * np.maximum(1.0, T_ref)), (T_ref, T[0, sub])
