@@ -54,6 +54,7 @@ def parse():
     ap.add_argument("--n-E", type=int, default=512)
     ap.add_argument("--cohort", type=int, default=0)
     ap.add_argument("--form", default="half", choices=["half", "dense"], help="formulation of the sweep (include/rgf.h)")
+    ap.add_argument("--no-guard", action="store_true", help="switch the near-neutrality guard off (rgf_set_guard 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -203,6 +204,8 @@ def main():
     if a.cohort:
         rgf.rgf_set_cohort(plan, a.cohort)
     rgf.rgf_set_formulation(plan, rgf.RGF_FORM_HALF if a.form == "half" else rgf.RGF_FORM_DENSE)
+    if a.no_guard:
+        rgf.rgf_set_guard(plan, 0.0)
     peak = rgf.rgf_fp64_peak_tflops(plan)
     rgf.rgf_set_device(plan, w.M, w.L, onsite, w.t, None)
     E_dev = torch.from_numpy(E_host).to(dev)
@@ -291,8 +294,9 @@ def main():
             "energies_per_s": world * n_E * a.steps / (ms_max * 1e-3),
             "tflops_executed": flops_step * world * a.steps / (ms_max * 1e-3) * 1e-12,
             "tflops_dense_equivalent": 16.0 * w.M ** 3 * units_step * a.steps / (ms_max * 1e-3) * 1e-12,
-            "phase_ms_last_step": {k: stats[k] for k in ("ms_total", "ms_leads", "ms_sweep", "ms_trace", "ms_inverse_update")},
+            "phase_ms_last_step": {k: stats[k] for k in ("ms_total", "ms_leads", "ms_sweep", "ms_trace", "ms_inverse_update", "ms_guard")},
             "lead_iterations": stats["lead_iterations"],
+            "guard_redone_energies": stats["guard_redone"],
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": peak,

@@ -100,6 +100,7 @@ typedef struct rgf_stats {
     int cohort;                 /* matrices per launch                                           */
     int guard_redone;           /* energies recomputed in RGF_FORM_DENSE by the near-neutrality guard */
     int reserved;
+    double ms_guard;            /* of ms_total: the guard's second pass (leads + dense sweep + trace of the redone energies) */
 } rgf_stats;
 int rgf_get_stats(const rgf_plan *p, rgf_stats *out);
 
@@ -140,14 +141,17 @@ int rgf_set_lead_method(rgf_plan *p, int method);
 
 /* Near-charge-neutrality guard of RGF_FORM_HALF (complex128, fused kernel).  The cut between the two halves of a slice
  * leaves singly bonded atoms whose edge-like states are resonant close to charge neutrality (PAPER.md:82 is about
- * exactly this energy range); a step then loses about 0.2 eps_mach (|t| max|g|)^2.  The fused kernel records the
- * smallest pivot of every (device, energy) pair, G = |t| / min|pivot|, and every energy with
- *     2.4e-17 G^2 T / max(1, T) > tol
- * for some device is computed again in RGF_FORM_DENSE, which has no such cut, inside the same rgf_transmission call.
- * tol = 0 switches the guard off; default 3e-11.  rgf_stats.guard_redone counts the energies recomputed. */
+ * exactly this energy range); a B half-step with smallest pivot p loses about eps_mach (|t| / p)^2.  The fused
+ * kernel records that pivot for every B half-step of every (device, energy) pair; with G the root mean square of
+ * |t| / p over the L B half-steps (in a clean ribbon every half-step has the same p), every energy with
+ *     1.5e-16 G^2 min(1, T) > tol
+ * for some device is computed again in RGF_FORM_DENSE, which has no such cut, inside the same rgf_transmission call
+ * (the constant is calibrated in DESIGN.md section 1a).  tol = 0 switches the guard off; default 1e-10, a tenth of the
+ * tolerance 1e-9 max(1, T).  rgf_stats.guard_redone counts the energies recomputed. */
 int rgf_set_guard(rgf_plan *p, double tol);
-/* G of the first pass of the last rgf_transmission call, [n_dev][n_E] (HOST pointer; 0 where not recorded). */
-int rgf_get_guard_indicators(const rgf_plan *p, double *G_out, int n);
+/* Indicators of the first pass of the last rgf_transmission call, [n_dev][n_E] each (HOST pointers; 0 where not
+ * recorded): Grms_out = G above, Gmax_out (may be NULL) = |t| / (smallest pivot of the whole sweep). */
+int rgf_get_guard_indicators(const rgf_plan *p, double *Grms_out, double *Gmax_out, int n);
 
 /* Matrices per kernel launch in the sweep (0 = library default).  RGF_FORM_DENSE / _STEPWISE and the complex64 sweep:
  * the sweep runs cohort after cohort over all slices.  RGF_FORM_HALF in complex128 (fused kernel): the whole batch is one

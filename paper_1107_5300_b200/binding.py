@@ -27,7 +27,7 @@ _lib = C.CDLL(LIB_PATH)
 class rgf_stats(C.Structure):
     _fields_ = [("ms_total", C.c_double), ("ms_leads", C.c_double), ("ms_sweep", C.c_double), ("ms_trace", C.c_double),
                 ("ms_inverse_update", C.c_double), ("launches", C.c_longlong), ("launches_inverse_update", C.c_longlong), ("launches_leads", C.c_longlong),
-                ("lead_iterations", C.c_int), ("cohort", C.c_int), ("guard_redone", C.c_int), ("reserved", C.c_int)]
+                ("lead_iterations", C.c_int), ("cohort", C.c_int), ("guard_redone", C.c_int), ("reserved", C.c_int), ("ms_guard", C.c_double)]
 
 
 _vp = C.c_void_p
@@ -44,7 +44,7 @@ _lib.rgf_set_cohort.argtypes = [_vp, C.c_int]
 _lib.rgf_set_formulation.argtypes = [_vp, C.c_int]
 _lib.rgf_set_lead_method.argtypes = [_vp, C.c_int]
 _lib.rgf_set_guard.argtypes = [_vp, C.c_double]
-_lib.rgf_get_guard_indicators.argtypes = [_vp, _vp, C.c_int]
+_lib.rgf_get_guard_indicators.argtypes = [_vp, _vp, _vp, C.c_int]
 _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
@@ -132,8 +132,8 @@ def rgf_set_guard(plan, tol):
     return _check(plan, _lib.rgf_set_guard(plan, tol))
 
 
-def rgf_get_guard_indicators(plan, G_out, n):
-    return _check(plan, _lib.rgf_get_guard_indicators(plan, _addr(G_out, np.float64), n))
+def rgf_get_guard_indicators(plan, Grms_out, Gmax_out, n):
+    return _check(plan, _lib.rgf_get_guard_indicators(plan, _addr(Grms_out, np.float64), _addr(Gmax_out, np.float64), n))
 
 
 def rgf_fp64_peak_tflops(plan):

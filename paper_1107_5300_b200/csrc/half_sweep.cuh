@@ -44,7 +44,8 @@ struct HSweepArgs {
     cplx *X0, *X1, *P0, *P1;      // [nb][ldn*ldn] each
     int *perm;                    // [nb][2][HS_NMAX]: row and column maps of a matrix between launches
     int *status;                  // [nb]
-    unsigned *pivmin;             // [nb] or NULL: min over all pivots of the top 24 bits of max(|re|, |im|) (near-neutrality guard)
+    unsigned *pivmin;             // [nb] or NULL: min over all pivots of the top 24 bits of max(|re|, |im|)
+    double *gsq;                  // [nb] (with pivmin): sum over the B half-steps of 1 / (smallest pivot)^2   (near-neutrality guard)
     int hs_begin, hs_end;         // half-steps [begin, end) of the whole sweep: hs = 2 i + kind
     int unit0, unit_len;          // this launch runs units unit0 + blockIdx.x; unit u = (matrix u % nb, half-steps
                                   // [hs_begin + (u / nb) unit_len, + unit_len)): rounds of units keep every CTA slot busy
@@ -746,7 +747,8 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
     cplx *const X0 = a.X0 + bl * xs, *const X1 = a.X1 + bl * xs, *const W0 = a.P0 + bl * xs, *const W1 = a.P1 + bl * xs;
     int *gmaps = a.perm + (long long)bl * 2 * HS_NMAX;
     int *status_slot = a.status + bl;
-    if (tid == 0) sm.pivmin = 0xffffffffu;
+    unsigned kmin = 0xffffffffu;          // thread 0: smallest pivot key of the unit, and the guard's sum
+    double gsq = 0.0;
     if (hs_begin > 0) {
         if (tid < HS_NMAX) { sm.rmap[tid] = gmaps[tid]; sm.cmap[tid] = gmaps[HS_NMAX + tid]; }
         __syncthreads();
@@ -764,6 +766,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         const int par = kind == 0 ? ((i + 1) & 1) : (i & 1);
         n = half_count(M, par);
         if (tid < HS_NMAX) { sm.rmap_prev[tid] = sm.rmap[tid]; sm.cmap_prev[tid] = sm.cmap[tid]; }
+        if (tid == 0) sm.pivmin = 0xffffffffu;
         __syncthreads();
         if (inplace) {
             // tables of the in-place assembly (HSXf): atom r of this B half sits in physical row rmap[r] and its column
@@ -797,6 +800,11 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
         // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
         // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].
+        if (tid == 0) {
+            const unsigned km = sm.pivmin;
+            kmin = min(kmin, km);
+            if (kind == 0 && km != 0xffffffffu) { const double pm = __hiloint2double((int)(km << 8), 0); gsq += 1.0 / (pm * pm); }
+        }
         if (tid < n) {
             const int g0 = inplace ? sm.cmap_prev[tid] : tid, r0 = inplace ? sm.rmap_prev[tid] : tid;
             sm.rmap[tid] = sm.perm[g0];
@@ -805,7 +813,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         __syncthreads();
     }
     if (tid < HS_NMAX) { gmaps[tid] = sm.rmap[tid]; gmaps[HS_NMAX + tid] = sm.cmap[tid]; }
-    if (tid == 0 && a.pivmin) atomicMin(a.pivmin + bl, sm.pivmin);
+    if (tid == 0 && a.pivmin) { atomicMin(a.pivmin + bl, kmin); atomicAdd(a.gsq + bl, gsq); }
     if (hs_end == a.hs_end && (a.g_out || a.P_out)) {
         const int fb = hs_out_buf(hs_end - 1);
         const cplx *Xf = fb ? X1 : X0, *Wf = fb ? W1 : W0;

@@ -60,9 +60,9 @@ struct rgf_plan {
     double t = 0.0;
     Buf onsite, bond, hop, bondc;                 // device description
     Buf E, T, status, lead_flags;                 // per call
-    Buf pivmin, T_keep, redo_idx;                 // near-neutrality guard: smallest pivot per matrix, first-pass T, redone energies
-    std::vector<double> guard_G;                  // |t| / smallest pivot per batch item of the last call
-    double guard_tol = 3e-11;
+    Buf pivmin, gsq, T_keep, redo_idx;                 // near-neutrality guard: smallest pivot per matrix, first-pass T, redone energies
+    std::vector<double> guard_G, guard_Gmax;      // rms over the B half-steps / max of |t| / smallest pivot, per batch item of the last call
+    double guard_tol = 1e-10;
     std::vector<Ws> ws;                           // ws[0] runs on the plan's stream
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
@@ -308,6 +308,7 @@ namespace {
 //     K[r][c] = t^2 * #(atoms adjacent to both corner atoms r and c): 8x fewer flops; resonant only at E = +-t, where
 //     the caller takes the dense route.  The inverse of S gets one Newton step (the decimation amplifies its residual).
 // ------------------------------------------------------------------------------------------
+constexpr double kGuardC = 1.5e-16;        // estimated |dT| of the half-slice cut = kGuardC G_rms^2 min(1, T)
 constexpr double kLeadTol = 1e-14;
 constexpr int kLeadMaxIt = 64;
 
@@ -632,6 +633,7 @@ int run_sweep_cohort_fused(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int
     a.gL = ptr<cplx>(p->gL); a.gR = lead_gR(p);
     a.status = ptr<int>(p->status) + bz0;
     a.pivmin = p->pivmin.p ? ptr<unsigned>(p->pivmin) + bz0 : nullptr;
+    a.gsq = p->gsq.p ? ptr<double>(p->gsq) + bz0 : nullptr;
     a.hs_begin = 0; a.hs_end = 2 * nslices;
     a.g_out = ptr<cplx>(w.H0); a.P_out = ptr<cplx>(w.Pa);
     if ((rc = fused_launch(p, w, a, nb))) return rc;
@@ -851,13 +853,15 @@ int rgf_set_device(rgf_plan *p, int M, int L, const double *onsite, double t, co
 // One pass of the hot path over the n_E energies in p->E: leads (A2), sweep (A3-A5) and trace (A6) in `formulation`.
 // Writes p->T [n_dev][n_E] (NaN where an energy failed), p->status, p->lead_flags / p->lead_status, and for the fused
 // kernel p->pivmin.  *lead_open = number of energies whose lead decimation did not converge.
-static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, int *lead_open_out)
+static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, int *lead_open_out, bool first_pass = true)
 {
     int rc;
     const int batch = p->n_dev * n_E;
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
     if ((rc = ensure(p, p->T, sizeof(double) * (size_t)batch))) return rc;
     if ((rc = ensure(p, p->pivmin, sizeof(unsigned) * (size_t)batch))) return rc;
+    if ((rc = ensure(p, p->gsq, sizeof(double) * (size_t)batch))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->gsq.p, 0, sizeof(double) * (size_t)batch, p->stream));
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
     CUDA_TRY(p, cudaMemsetAsync(p->pivmin.p, 0xff, sizeof(unsigned) * (size_t)batch, p->stream));
     const int saved_form = p->formulation;
@@ -873,12 +877,12 @@ static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, 
     CUDA_TRY(p, cudaEventRecord(p->ev[2], p->stream));
     // ---- sweep + trace, cohort after cohort
     const int cohort = choose_cohort(p, batch);
-    p->stats.cohort = cohort;
+    if (first_pass) p->stats.cohort = cohort;
     const bool half = formulation != RGF_FORM_DENSE;
     Ws &w = p->ws[0];
     if ((rc = half ? ensure_sweep_ws_half(p, w, cohort) : ensure_sweep_ws(p, w, cohort))) { p->formulation = saved_form; return rc; }
     nvtxRangePushA("rgf_sweep");
-    p->in_sweep = true;
+    p->in_sweep = first_pass;          // the dominant kernel's events and launch count describe the first pass only
     for (int bz0 = 0; bz0 < batch && rc == RGF_OK; bz0 += cohort) {
         const int nb = std::min(cohort, batch - bz0);
         cplx *G = nullptr, *Galt = nullptr, *Pcur = nullptr;
@@ -903,6 +907,7 @@ static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, 
     float ms = 0.f;
     cudaEventElapsedTime(&ms, p->ev[1], p->ev[2]); p->stats.ms_leads += ms;
     cudaEventElapsedTime(&ms, p->ev[2], p->ev[3]); p->stats.ms_sweep += ms;
+    if (!first_pass) { float m2 = 0.f; cudaEventElapsedTime(&m2, p->ev[1], p->ev[3]); p->stats.ms_guard += m2; }
     if (lead_open_out) *lead_open_out = lead_open;
     return RGF_OK;
 }
@@ -955,10 +960,12 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
     // ~ 0.2 eps_mach (|t| max|gB|)^2.  The fused kernel records the smallest pivot of every matrix; items whose estimate
     // exceeds guard_tol are computed again in RGF_FORM_DENSE (no such cut) and replace the first result.
     p->guard_G.assign(batch, 0.0);
+    p->guard_Gmax.assign(batch, 0.0);
     if (p->guard_tol > 0.0 && precision == RGF_C128 && use_fused(p)) {
         std::vector<unsigned> key(batch);
-        std::vector<double> hT(batch);
+        std::vector<double> hT(batch), gsq(batch);
         CUDA_TRY(p, cudaMemcpyAsync(key.data(), p->pivmin.p, sizeof(unsigned) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+        CUDA_TRY(p, cudaMemcpyAsync(gsq.data(), p->gsq.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
         CUDA_TRY(p, cudaMemcpyAsync(hT.data(), p->T.p, sizeof(double) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         std::vector<char> redo(n_E, 0);
@@ -966,10 +973,11 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
             const unsigned long long bits = ((unsigned long long)(key[b] << 8)) << 32;
             double piv;
             memcpy(&piv, &bits, sizeof(piv));
-            const double G = (key[b] == 0xffffffffu || !(piv > 0.0)) ? 0.0 : std::fabs(p->t) / piv;
+            p->guard_Gmax[b] = (key[b] == 0xffffffffu || !(piv > 0.0)) ? 0.0 : std::fabs(p->t) / piv;
+            const double G = std::fabs(p->t) * std::sqrt(gsq[b] / (double)p->L);       // rms over the L B half-steps
             p->guard_G[b] = G;
             const double T = std::isfinite(hT[b]) ? std::fabs(hT[b]) : 1.0;
-            if (2.4e-17 * G * G * T / std::max(1.0, T) > p->guard_tol) redo[b % n_E] = 1;
+            if (!(kGuardC * G * G * T / std::max(1.0, T) <= p->guard_tol)) redo[b % n_E] = 1;
         }
         std::vector<int> idx;
         std::vector<double> E2;
@@ -984,7 +992,7 @@ int rgf_transmission(rgf_plan *p, const double *energies, int n_E, double eta, i
             CUDA_TRY(p, cudaMemcpyAsync(p->E.p, E2.data(), sizeof(double) * (size_t)n2, cudaMemcpyHostToDevice, p->stream));
             CUDA_TRY(p, cudaStreamSynchronize(p->stream));          // idx / E2 are host vectors
             int open2 = 0;
-            if ((rc = transmission_pass(p, n2, eta, RGF_FORM_DENSE, &open2))) return rc;
+            if ((rc = transmission_pass(p, n2, eta, RGF_FORM_DENSE, &open2, false))) return rc;
             const int r2 = pass_result(p, n2, open2, RGF_OK);
             if (r2 != RGF_OK) result = r2;
             scatter_T_kernel<<<(p->n_dev * n2 + 255) / 256, 256, 0, p->stream>>>(ptr<double>(p->T_keep), ptr<double>(p->T), ptr<int>(p->redo_idx),
@@ -1010,7 +1018,7 @@ int rgf_destroy(rgf_plan *p)
     if (!p) return RGF_OK;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->pivmin, &p->T_keep, &p->redo_idx,
+    Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->pivmin, &p->gsq, &p->T_keep, &p->redo_idx,
                    &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3,
                    &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status};
     for (Buf *b : bufs) release(*b);
@@ -1065,10 +1073,13 @@ int rgf_set_guard(rgf_plan *p, double tol)
     return RGF_OK;
 }
 
-int rgf_get_guard_indicators(const rgf_plan *p, double *G_out, int n)
+int rgf_get_guard_indicators(const rgf_plan *p, double *Grms_out, double *Gmax_out, int n)
 {
-    if (!p || !G_out || n < 0) return RGF_EINVAL;
-    for (int k = 0; k < n; k++) G_out[k] = k < (int)p->guard_G.size() ? p->guard_G[k] : 0.0;
+    if (!p || !Grms_out || n < 0) return RGF_EINVAL;
+    for (int k = 0; k < n; k++) {
+        Grms_out[k] = k < (int)p->guard_G.size() ? p->guard_G[k] : 0.0;
+        if (Gmax_out) Gmax_out[k] = k < (int)p->guard_Gmax.size() ? p->guard_Gmax[k] : 0.0;
+    }
     return RGF_OK;
 }
 
@@ -1195,6 +1206,7 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
     CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
     if ((rc = ensure(p, p->pivmin, sizeof(unsigned) * (size_t)batch))) return rc;
+    if ((rc = ensure(p, p->gsq, sizeof(double) * (size_t)batch))) return rc;
     if ((rc = run_leads(p, n_E, eta, nullptr))) return rc;
     Ws &w = p->ws[0];
     const bool half = p->formulation != RGF_FORM_DENSE;

@@ -95,6 +95,30 @@ def config4(M=1024, L=2000, n_E=64, seed_onsite=5302, seed_vac=5303, W=0.1, prob
                     np.linspace(-0.5, 0.5, n_E), notes={"seeds": [seed_onsite, seed_vac], "W": W, "prob": prob})
 
 
+NEAR_NEUTRALITY_CASES = ("clean_M20", "clean_M20_vacancy", "disordered_M128", "disordered_M128_vacancy")
+
+
+def near_neutrality(case):
+    """Conducting (metallic: M + 1 divisible by 3) ribbons probed at |E| = 1e-2 ... 1e-5 eV, the edge case of the method
+    (PAPER.md:82): clean M = 20, L = 40 and Anderson +-0.25 eV M = 128, L = 200 (seed 4242), each also with two edge vacancies."""
+    assert case in NEAR_NEUTRALITY_CASES, case
+    if case.startswith("clean"):
+        M, L = 20, 40
+        on = np.zeros((L, M))
+    else:
+        M, L = 128, 200
+        on = anderson(M, L, 0.25, 4242)
+    vac = None
+    if case.endswith("vacancy"):
+        vac = np.zeros((L, M), dtype=np.uint8)
+        vac[L // 2, 0] = 1
+        vac[L // 3, M - 1] = 1
+        on = on.copy()
+        on[vac != 0] = VACANCY_ONSITE
+    E = np.array([s * e for e in (1e-2, 1e-3, 1e-4, 1e-5) for s in (1.0, -1.0)])
+    return Workload("near neutrality " + case, M, L, on[None], None if vac is None else vac[None], E)
+
+
 def truncate(w: Workload, L: int, energy_index=None) -> Workload:
     """First L slices of the same arrays (leads then attach at slice L) and a subset of energies."""
     E = w.energies if energy_index is None else w.energies[np.asarray(energy_index)]

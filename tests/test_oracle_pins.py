@@ -326,3 +326,40 @@ def test_generators_are_seeded_and_shaped():
     w3 = inputs.config3(L=4)
     assert w3.n_E == 1024 and w3.energies[0] == -1.0 and w3.energies[511] == 1.0 and abs(w3.energies[512] + 0.05) < 1e-15
     assert 0.0 not in w3.energies            # even counts never sample E = 0 (Q7)
+
+
+# ----------------------------------------------------------------------------------------
+# The 80-bit evaluator behind tests/golden/near_neutrality_ld.txt (neither oracle nor CUDA), pinned both ways
+# ----------------------------------------------------------------------------------------
+
+def test_extended_precision_evaluator_matches_oracle_and_closed_form(oracle):
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_near_neutrality_ld", os.path.join(GOLDEN, "make_near_neutrality_ld.py"))
+    ld = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(ld)
+    # disordered, vacancies, odd M and odd L, away from E = 0: the oracle is accurate there
+    M, L = 9, 7
+    on = inputs.anderson(M, L, 0.3, 31)
+    vac = np.zeros((L, M), dtype=np.uint8)
+    vac[0, 1] = vac[3, 0] = vac[L - 1, 4] = 1
+    for E in (-1.3, 0.21, 0.9):
+        T_or = oracle.transmission_batch(on, vac, T_HOP, np.array([E]), ETA)[0]
+        assert abs(ld.transmission_ld(on, vac, T_HOP, E, ETA) - T_or) < 1e-11, E
+    # clean metallic ribbon at |E| = 1e-5 eV: closed form
+    M, L = 8, 6
+    Tc = closed_form_T(M, L, 1e-5)[0]
+    assert abs(ld.transmission_ld(np.zeros((L, M)), None, T_HOP, 1e-5, ETA) - Tc) < 1e-13
+
+
+def test_near_neutrality_golden_is_consistent_with_the_oracle(oracle):
+    """Stored 80-bit values vs the oracle: equal to 1e-9 where the oracle is accurate (|E| >= 1e-3 eV), and within the
+    oracle's documented loss (< 1e-7) below."""
+    path = os.path.join(GOLDEN, "near_neutrality_ld.txt")
+    rows = [l.split() for l in open(path) if not l.startswith("#")]
+    assert len(rows) == 32
+    for case in ("clean_M20", "clean_M20_vacancy"):
+        w = inputs.near_neutrality(case)
+        vac = None if w.vacancy is None else w.vacancy[0]
+        T_or = oracle.transmission_batch(w.onsite[0], vac, w.t, w.energies, w.eta)
+        T_ld = np.array([float(r[3]) for r in rows if r[0] == case])
+        assert np.all(np.abs(T_or - T_ld) <= 1e-9), (case, np.abs(T_or - T_ld))
