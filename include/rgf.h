@@ -183,6 +183,29 @@ int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, 
 int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int precision,
                     int nslices, double *g_out, double *P_out);
 
+/* ---- allocation-free entry point --------------------------------------------------------------------------
+ * A4 alone like rgf_inverse_batched (same kernels, n <= 256 path), for callers that cannot call cudaMalloc: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid allocation.  It takes no plan and calls no cudaMalloc, cudaFree
+ * or other allocating routine: all scratch (two work copies of the batch, the panel multipliers, the row maps, the pivot
+ * flags) lives in one file-scope __device__ array of RGF_STATIC_SCRATCH_MB that every GPU loading the library holds until exit.
+ *   cuda_device / cuda_stream   device ordinal and cudaStream_t (NULL = default stream) the work is enqueued on
+ *   A_dev, Ainv_dev             DEVICE pointers on that device: batch complex n x n matrices, interleaved re,im doubles,
+ *                               row-major, matrix b at + b*n*n*2 doubles.  A_dev is not modified; Ainv_dev may equal A_dev.
+ *   status_dev                  DEVICE pointer to batch ints or NULL: 1 where a pivot was zero / non-finite, else 0.
+ * Asynchronous: results are valid once the stream has completed the call.  Limits: n <= RGF_STATIC_MAX_N,
+ * batch <= RGF_STATIC_MAX_BATCH, n*n*batch <= RGF_STATIC_MAX_ELEMS, n*batch <= 64*RGF_STATIC_MAX_BATCH; anything larger
+ * returns RGF_EUNSUPPORTED (message: rgf_static_last_error) -- use rgf_inverse_batched.  Host pointers return RGF_EINVAL.
+ * Every call on a device shares the one array, which keeps the last call's contents (the call clears what must start
+ * at zero): two calls that overlap on the GPU -- different streams, or two host threads -- RACE; serialise them on one
+ * stream or with events.  The array's address is resolved once per device (cudaGetSymbolAddress with that device current). */
+#define RGF_STATIC_MAX_N 256
+#define RGF_STATIC_MAX_BATCH 64
+#define RGF_STATIC_MAX_ELEMS 262144
+#define RGF_STATIC_SCRATCH_MB 10.04
+int rgf_inverse_batched_static(int cuda_device, void *cuda_stream, int n, int batch, const double *A_dev, double *Ainv_dev,
+                               int *status_dev);
+const char *rgf_static_last_error(void);     /* message of the last failed rgf_inverse_batched_static call of this thread */
+
 #ifdef __cplusplus
 }
 #endif

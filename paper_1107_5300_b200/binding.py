@@ -49,6 +49,8 @@ _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
 _lib.rgf_sweep_state.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, C.c_int, _vp, _vp]
+_lib.rgf_inverse_batched_static.argtypes = [C.c_int, _vp, C.c_int, C.c_int, _vp, _vp, _vp]
+_lib.rgf_static_last_error.restype = C.c_char_p
 
 
 class RgfError(RuntimeError):
@@ -154,6 +156,18 @@ def rgf_lead_self_energy(plan, dev, energies, n_E, eta, side, Sigma_out):
 
 def rgf_sweep_state(plan, dev, energies, n_E, eta, precision, nslices, g_out, P_out):
     return _check(plan, _lib.rgf_sweep_state(plan, dev, _addr(energies), n_E, eta, precision, nslices, _addr(g_out), _addr(P_out)))
+
+
+def rgf_static_last_error():
+    return _lib.rgf_static_last_error().decode()
+
+
+def rgf_inverse_batched_static(cuda_device, cuda_stream, n, batch, A_dev, Ainv_dev, status_dev=None):
+    """Allocation-free inverse (include/rgf.h): device tensors in and out, scratch in the library's static array."""
+    rc = _lib.rgf_inverse_batched_static(cuda_device, cuda_stream, n, batch, _addr(A_dev), _addr(Ainv_dev), _addr(status_dev))
+    if rc != RGF_OK:
+        raise RgfError(rc, rgf_static_last_error())
+    return rc
 
 
 class Plan:

@@ -15,6 +15,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/rgf.h"
@@ -1229,6 +1230,117 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     CUDA_TRY(p, cudaMemcpyAsync(P_out, p->stage_out.p, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     drain_update_events(p);
+    return RGF_OK;
+}
+
+}  // extern "C"
+
+// ==========================================================================================
+// Allocation-free entry point: rgf_inverse_batched_static (include/rgf.h).  A4 alone -- the n <= 256 path of
+// run_inverse (gj32_panel_kernel / gj32_update_kernel / gj32_unpermute_kernel, the same kernels) -- with every byte of
+// scratch in ONE file-scope device array, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving
+// loops, harnesses that forbid it).  It takes no plan (a plan owns streams, events and buffers) and calls no cudaMalloc /
+// cudaFree / allocating library routine.  Every GPU that loads the library holds the array until exit.
+// ==========================================================================================
+#define RGF_STATIC_SCRATCH_BYTES (2ull * RGF_STATIC_MAX_ELEMS * 16 + (unsigned long long)RGF_STATIC_MAX_BATCH * 64 * 32 * 16 \
+                                  + 2ull * RGF_STATIC_MAX_BATCH * 64 * 4 + 4096)
+static __device__ __align__(256) unsigned char rgf_static_scratch[RGF_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticSetup { bool done; unsigned char *base; };
+StaticSetup g_static[kStaticMaxDevices];
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_static_err, sizeof(g_static_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+// once per device, with that device current: the DEVICE address of the scratch array (in host code the array's name is
+// only a stand-in) and the shared-memory attributes of the two kernels that need more than 48 KB
+int static_setup(int dev, unsigned char **base)
+{
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!g_static[dev].done) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, rgf_static_scratch);
+        if (e != cudaSuccess || !ptr) return static_fail(RGF_ECUDA, "cudaGetSymbolAddress(rgf_static_scratch) failed on device %d: %s", dev, cudaGetErrorString(e));
+        if ((e = cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256))) != cudaSuccess ||
+            (e = cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM)) != cudaSuccess)
+            return static_fail(RGF_ECUDA, "cudaFuncSetAttribute failed on device %d: %s", dev, cudaGetErrorString(e));
+        g_static[dev].base = static_cast<unsigned char *>(ptr);
+        g_static[dev].done = true;
+    }
+    *base = g_static[dev].base;
+    return RGF_OK;
+}
+
+bool is_device_pointer(const void *p, int dev)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) && at.device == dev;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *rgf_static_last_error(void) { return g_static_err; }
+
+int rgf_inverse_batched_static(int cuda_device, void *cuda_stream, int n, int batch, const double *A_dev, double *Ainv_dev, int *status_dev)
+{
+    g_static_err[0] = 0;
+    if (n < 1 || batch < 1 || !A_dev || !Ainv_dev) return static_fail(RGF_EINVAL, "rgf_inverse_batched_static: need n >= 1, batch >= 1, A_dev and Ainv_dev non-NULL");
+    if (n > RGF_STATIC_MAX_N || batch > RGF_STATIC_MAX_BATCH || (long long)n * n * batch > RGF_STATIC_MAX_ELEMS || (long long)n * batch > 64LL * RGF_STATIC_MAX_BATCH)
+        return static_fail(RGF_EUNSUPPORTED, "rgf_inverse_batched_static: n = %d, batch = %d exceeds the static scratch (n <= %d, batch <= %d, n*n*batch <= %d, n*batch <= %d); "
+                           "use rgf_inverse_batched", n, batch, RGF_STATIC_MAX_N, RGF_STATIC_MAX_BATCH, RGF_STATIC_MAX_ELEMS, 64 * RGF_STATIC_MAX_BATCH);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev || cuda_device >= kStaticMaxDevices)
+        return static_fail(RGF_ECUDA, "rgf_inverse_batched_static: no CUDA device %d", cuda_device);
+    cudaError_t e;
+    if ((e = cudaSetDevice(cuda_device)) != cudaSuccess) return static_fail(RGF_ECUDA, "cudaSetDevice(%d): %s", cuda_device, cudaGetErrorString(e));
+    if (!is_device_pointer(A_dev, cuda_device) || !is_device_pointer(Ainv_dev, cuda_device) || (status_dev && !is_device_pointer(status_dev, cuda_device)))
+        return static_fail(RGF_EINVAL, "rgf_inverse_batched_static: A_dev, Ainv_dev and status_dev must be device pointers on device %d", cuda_device);
+    unsigned char *base = nullptr;
+    int rc = static_setup(cuda_device, &base);
+    if (rc) return rc;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    // carve the array: two n x n work buffers per matrix, the multipliers of a panel, the two row maps, the flags
+    const long long gb = (long long)n * n;
+    cplx *X = reinterpret_cast<cplx *>(base);
+    cplx *Y = X + RGF_STATIC_MAX_ELEMS;
+    cplx *Mult = Y + RGF_STATIC_MAX_ELEMS;
+    int *rowAt = reinterpret_cast<int *>(Mult + (size_t)RGF_STATIC_MAX_BATCH * 64 * 32);
+    int *orig = rowAt + RGF_STATIC_MAX_BATCH * 64;
+    int *status = orig + RGF_STATIC_MAX_BATCH * 64;
+    // the array keeps the last call's contents: the flags must start at zero, orig at the identity; X, Mult, rowAt are
+    // fully written before they are read, Y only ever holds what this call's panels and updates wrote
+    if ((e = cudaMemsetAsync(status, 0, sizeof(int) * (size_t)batch, stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(X, A_dev, sizeof(cplx) * (size_t)gb * batch, cudaMemcpyDeviceToDevice, stream)) != cudaSuccess)
+        return static_fail(RGF_ECUDA, "rgf_inverse_batched_static: %s", cudaGetErrorString(e));
+    const int total = n * batch;
+    gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, stream>>>(orig, n, total);
+    for (int k0 = 0; k0 < n; k0 += G32_B) {
+        gj32_panel_kernel<<<batch, G32_NT, gj32_panel_smem(n), stream>>>(X, Y, gb, n, k0, Mult, rowAt, orig, status);
+        if (n > G32_B) {
+            dim3 grid((n + GU32_BN - 1) / GU32_BN, (n + GU32_BM - 1) / GU32_BM, batch);
+            gj32_update_kernel<<<grid, GU32_THREADS, GU32_SMEM, stream>>>(X, Y, gb, n, k0, Mult, rowAt);
+        }
+        std::swap(X, Y);
+    }
+    dim3 grid((n + 7) / 8, batch);
+    gj32_unpermute_kernel<<<grid, 256, 0, stream>>>(X, reinterpret_cast<cplx *>(Ainv_dev), gb, n, orig);
+    if (status_dev && (e = cudaMemcpyAsync(status_dev, status, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToDevice, stream)) != cudaSuccess)
+        return static_fail(RGF_ECUDA, "rgf_inverse_batched_static: %s", cudaGetErrorString(e));
+    if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(RGF_ECUDA, "rgf_inverse_batched_static: launch failed: %s", cudaGetErrorString(e));
     return RGF_OK;
 }
 
