@@ -5,7 +5,7 @@ configs[3] in complex128 and in complex64 through the C ABI and reports |T_c64 -
 maximum per energy window and the growth towards charge neutrality that north_star asks to be reported.
 Marshalling and a table only -- every number comes from the CUDA library.
 
-    python -m paper_1107_5300_b200.precision_study [--L 2000] [--out profiles/precision_r01_config3.md]
+    python -m paper_1107_5300_b200.precision_study [--L 2000] [--out profiles/precision_r02_config3.md]
 """
 import argparse
 import sys
