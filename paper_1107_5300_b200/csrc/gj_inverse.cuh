@@ -187,7 +187,8 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
 
 // ------------------------------------------------------------------------------------------
 // Trailing update on the FP64 tensor pipe: G[:,J] += Nbuf (n x B) * Rbuf[:,J] (B x |J|).
-// CTA = 4 warps stacked on rows: tile 128 rows x 32 columns; the accumulators are initialised
+// CTA = 4 warps stacked on rows: tile 128 rows x 32 columns; the Mult and pivot-row tiles are staged by TMA bulk copies
+// (cp.async.bulk + mbarrier: BASELINE.json north_star "Large M uses TMA-staged panels"); the accumulators are initialised
 // from G and stored back in place (each element is read and written by exactly one lane).
 // 8-column blocks inside the panel [k0, k0+B) are skipped.
 // ------------------------------------------------------------------------------------------
@@ -215,17 +216,17 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
     if (col0 >= k0 && col0 + GU_BN <= k0 + B) return;
     static_assert(B % 4 == 0, "panel width must be a multiple of the DMMA k");
 
-    for (int e = tid; e < GU_BM * B; e += GU_THREADS) {
-        int rr = e / B, k = e % B;
-        bool ok = row0 + rr < n;
-        cp_async16(sN + rr * LDN + k, ok ? Nbuf + (long long)(row0 + rr) * B + k : Nbuf, ok ? 16 : 0);
-    }
-    for (int e = tid; e < B * GU_BN; e += GU_THREADS) {
-        int k = e / GU_BN, c = e % GU_BN;
-        bool ok = col0 + c < n;
-        cp_async16(sR + k * GU_LDR + c, ok ? Rbuf + (long long)k * n + col0 + c : Rbuf, ok ? 16 : 0);
-    }
-    cp_async_commit();
+    // stage Mult (rows row0 .., B columns: one contiguous row of the panel buffer each) and the B pivot rows (32 columns
+    // from col0) with TMA bulk copies; rows / columns beyond n are not loaded (they only feed accumulators that are never stored)
+    __shared__ unsigned long long bar;
+    const int nrows = (n - row0 < GU_BM) ? (n - row0) : GU_BM, ncolsR = (n - col0 < GU_BN) ? (n - col0) : GU_BN;
+    if (tid == 0) tma_bar_init(&bar, 1);
+    __syncthreads();
+    if (tid == 0) tma_expect(&bar, (unsigned)(nrows * B + B * ncolsR) * (unsigned)sizeof(cplx));
+    for (int rr = tid; rr < nrows; rr += GU_THREADS)
+        tma_load_row(sN + rr * LDN, Nbuf + (long long)(row0 + rr) * B, B * (unsigned)sizeof(cplx), &bar);
+    for (int k = tid; k < B; k += GU_THREADS)
+        tma_load_row(sR + k * GU_LDR, Rbuf + (long long)k * n + col0, ncolsR * (unsigned)sizeof(cplx), &bar);
 
     const int wr = row0 + warp * 32;
     int mb_valid = (n - wr + 7) / 8; mb_valid = mb_valid < 0 ? 0 : (mb_valid > 4 ? 4 : mb_valid);
@@ -247,8 +248,7 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
                 cre[i][j][q] = v.x; cim[i][j][q] = v.y;
             }
         }
-    cp_async_wait<0>();
-    __syncthreads();
+    tma_wait(&bar, 0);
     const cplx *cA = sN + warp * 32 * LDN;
 #pragma unroll
     for (int kk = 0; kk < B; kk += 4) {

@@ -63,6 +63,7 @@ struct HSmem {
     int rmap_prev[HS_NMAX], cmap_prev[HS_NMAX];
     int prow[HS_B];
     unsigned pivmin;
+    alignas(8) unsigned long long bar;                // mbarrier of the panel's TMA bulk copies
     // in-place assembly of a kind-B half-step (HSXf), per physical row / column of the previous result
     double xf_sr[HS_NMAX], xf_sw[HS_NMAX], xf_dre[HS_NMAX], xf_mc[HS_NMAX];
     short xf_dcol[HS_NMAX], xf_pa[HS_NMAX], xf_pb[HS_NMAX];
@@ -489,7 +490,7 @@ __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *pr
 // that HSXf turns into A while panel 0 is loaded and applied (xtf = 1); W likewise: wtf = 0 (W in place), 2 (previous
 // propagator, scaled in place) or 3 (stencil of the previous propagator in the other buffer) ---------------------------------------
 __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int ld, int n, int nc, int *status_slot,
-                                                int xtf, int wtf, const HSXf &xf)
+                                                int xtf, int wtf, const HSXf &xf, unsigned &tma_phase)
 {
     const int tid = threadIdx.x;
     bool used = !(tid < n);
@@ -500,13 +501,18 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
         const int bw = (n - k0 < HS_B) ? (n - k0) : HS_B;
         const bool tf = (xtf | wtf) != 0 && k0 == 0;
         if (!(tf && xtf)) {
-            for (int e = tid; e < HS_NMAX * HS_B; e += HS_NT) {
-                const int rr = e / HS_B, c = e % HS_B;
-                const bool ok = rr < n && c < bw;
-                cp_async16(sm.panel + rr * HS_LDP + c, ok ? X + (long long)rr * ld + k0 + c : X, ok ? 16 : 0);
+            // the n x bw panel by TMA: one bulk copy per row (bw contiguous elements of X), all completing on one mbarrier;
+            // the padding (rows >= n, columns >= bw) is zeroed with plain stores, which touch none of the copied bytes
+            if (tid == 0) tma_expect(&sm.bar, (unsigned)(n * bw) * (unsigned)sizeof(cplx));
+            if (tid < n) {
+                tma_fence_proxy();          // this buffer was last written / read through the generic proxy
+                tma_load_row(sm.panel + tid * HS_LDP, X + (long long)tid * ld + k0, (unsigned)bw * (unsigned)sizeof(cplx), &sm.bar);
+                for (int c = bw; c < HS_B; c++) sm.panel[tid * HS_LDP + c] = cmake(0.0, 0.0);
+            } else if (tid < HS_NMAX) {
+                for (int c = 0; c < HS_B; c++) sm.panel[tid * HS_LDP + c] = cmake(0.0, 0.0);
             }
-            cp_async_commit();
-            cp_async_wait<0>();
+            tma_wait(&sm.bar, tma_phase);
+            tma_phase ^= 1u;
         } else {
             // panel 0 of an in-place half-step: transformed on its way to shared memory, 8 loads in flight per thread
             constexpr int PER = 8;
@@ -748,6 +754,8 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
     int *gmaps = a.perm + (long long)bl * 2 * HS_NMAX;
     int *status_slot = a.status + bl;
     unsigned kmin = 0xffffffffu;          // thread 0: smallest pivot key of the unit, and the guard's sum
+    unsigned tma_phase = 0u;
+    if (tid == 0) tma_bar_init(&sm.bar, 1);
     double gsq = 0.0;
     if (hs_begin > 0) {
         if (tid < HS_NMAX) { sm.rmap[tid] = gmaps[tid]; sm.cmap[tid] = gmaps[HS_NMAX + tid]; }
@@ -796,7 +804,7 @@ __global__ void __launch_bounds__(HS_NT, 2) half_sweep_kernel(HSweepArgs a)
         }
         __syncthreads();
         xf.Wp = Wp;
-        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf);
+        hs_gauss_jordan(sm, Xn, Wn, ld, n, nc, status_slot, inplace ? 1 : 0, inplace ? 2 : (hs == 0 ? 0 : 3), xf, tma_phase);
         // maps of the new result.  The elimination ran on A' = A[rl(rho)][cl(gamma)] (rl, cl = identity for an assembled A,
         // the inverse maps of the previous result for an in-place one) and left (A'^-1)[gamma][rho'] at physical
         // (perm[gamma], pinv[rho']); (A'^-1)[gamma][rho'] = (A^-1)[cl(gamma)][rl(rho')].

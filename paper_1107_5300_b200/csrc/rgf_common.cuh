@@ -65,6 +65,40 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src,
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// ---- TMA bulk copies (cp.async.bulk, SASS: UBLKCP) completing on an mbarrier (SASS: SYNCS) ---------------------------
+// One elected thread arms the barrier with the byte count of the whole stage (tma_expect), any thread issues row copies
+// (16-byte aligned source, destination and size), every consumer waits on the phase parity (tma_wait).  The copy engine
+// moves the rows; no thread spends registers or address arithmetic per 16 bytes as with cp.async.
+__device__ __forceinline__ void tma_bar_init(unsigned long long *bar, int arrivals)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(arrivals) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tma_expect(unsigned long long *bar, unsigned bytes)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_row(void *smem_dst, const void *gmem_src, unsigned bytes, unsigned long long *bar)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(d), "l"(gmem_src), "r"(bytes), "r"(a) : "memory");
+}
+__device__ __forceinline__ void tma_wait(unsigned long long *bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "TMA_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra TMA_WAIT_%=;\n\t}"
+        ::"r"(a), "r"(parity) : "memory");
+}
+// generic-proxy writes (st.shared) of a buffer must be ordered before the async proxy overwrites it
+__device__ __forceinline__ void tma_fence_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // m_i[j] = 1 iff (i + j) even; bit test so that negative (lead) slice indices work
 __host__ __device__ __forceinline__ int mask_bit(int i, int j) { return (((i + j) & 1) == 0) ? 1 : 0; }
 
