@@ -28,6 +28,8 @@
  *
  * Complex arrays cross this ABI as interleaved (re,im) doubles, row-major.
  *
+ * orc_ldos_batch (O9) adds the diagonal blocks of the connected G (local density of states).
+ *
  * parity pins (tests/test_oracle_pins.py): closed-form subband transmission of the clean
  * ribbon, brute-force inversion of the whole device (orc_transmission_brute), reciprocity
  * (orc_transmission with direction=1), bipartite / gauge symmetries, lead fixed-point
@@ -522,6 +524,65 @@ static int brute(int M, int L, const double *onsite, const uint8_t *vac, double 
     return rc;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * O9. Local density of states of the connected device.
+ * PAPER.md:37 "Knowledge of the Green's function allows one to compute any desired quantity, e.g.
+ * charge density"; PAPER.md:61 (step 5: the Green's functions of the whole region).  Definition:
+ *   LDOS(i, j; E) = -(1/pi) Im G_ii[j][j],   G = (z - H_device - Sigma_L (+) 0 (+) Sigma_R)^-1  (Eq. 1)
+ * computed by the textbook two-pass recursion for the diagonal blocks (Dyson's equation, Eq. 3,
+ * applied from the right after the left-to-right sweep of Eq. 4):
+ *   forward   g_i = (z - H_i - V g_{i-1} V [- Sigma_L at 0] [- Sigma_R at L-1])^-1, all g_i kept
+ *   backward  G_{L-1,L-1} = g_{L-1};   G_ii = g_i + g_i V G_{i+1,i+1} V g_i,  V = t diag(m'_i)
+ * The brute-force pin (the definition itself, by numpy on a matrix the test assembles) is in
+ * tests/test_oracle_pins.py.  ldos_out[L][M].
+ * ---------------------------------------------------------------------------------------- */
+static int ldos_sweep(int M, int L, const double *onsite, const uint8_t *vac, double t, double E, double eta,
+                      int lead_method, double *ldos_out)
+{
+    const double pi = 3.14159265358979323846;
+    size_t MM = (size_t)M * M;
+    cplx z = c_make(E, eta);
+    cplx *gall = (cplx *)malloc(sizeof(cplx) * MM * (size_t)L);
+    cplx *buf = (cplx *)malloc(sizeof(cplx) * MM * 7);
+    double *mp = (double *)malloc(sizeof(double) * (size_t)M);
+    if (!gall || !buf || !mp) { free(gall); free(buf); free(mp); return ORC_ENOMEM; }
+    cplx *SigL = buf, *SigR = buf + MM, *A = buf + 2 * MM, *H = buf + 3 * MM, *G = buf + 4 * MM, *X = buf + 5 * MM, *Y = buf + 6 * MM;
+    int rc = lead_self_energy(M, L, vac, t, z, -1, lead_method, SigL, NULL);
+    if (rc == ORC_OK) rc = lead_self_energy(M, L, vac, t, z, +1, lead_method, SigR, NULL);
+    for (int i = 0; i < L && rc == ORC_OK; i++) {
+        slice_hamiltonian(M, L, onsite, vac, i, t, H);
+        for (size_t k = 0; k < MM; k++) A[k] = c_make(-H[k].re, -H[k].im);
+        for (int d = 0; d < M; d++) A[(size_t)d * M + d] = c_add(A[(size_t)d * M + d], z);
+        if (i == 0) for (size_t k = 0; k < MM; k++) A[k] = c_sub(A[k], SigL[k]);
+        if (i == L - 1) for (size_t k = 0; k < MM; k++) A[k] = c_sub(A[k], SigR[k]);
+        if (i > 0) {
+            bond_mask(M, L, vac, i - 1, mp);
+            const cplx *gp = gall + (size_t)(i - 1) * MM;
+            for (int r = 0; r < M; r++)
+                for (int c = 0; c < M; c++)
+                    A[(size_t)r * M + c] = c_sub(A[(size_t)r * M + c], c_scale(gp[(size_t)r * M + c], (t * mp[r]) * (t * mp[c])));
+        }
+        rc = mat_inverse(M, A, gall + (size_t)i * MM);
+    }
+    if (rc == ORC_OK) {
+        memcpy(G, gall + (size_t)(L - 1) * MM, sizeof(cplx) * MM);
+        for (int i = L - 1; i >= 0; i--) {
+            if (i < L - 1) {
+                const cplx *gi = gall + (size_t)i * MM;
+                bond_mask(M, L, vac, i, mp);
+                for (int r = 0; r < M; r++)                       /* V G_{i+1,i+1} V */
+                    for (int c = 0; c < M; c++) X[(size_t)r * M + c] = c_scale(G[(size_t)r * M + c], (t * mp[r]) * (t * mp[c]));
+                mat_mul(M, gi, X, Y);                               /* g_i V G V */
+                mat_mul(M, Y, gi, X);                               /* g_i V G V g_i */
+                for (size_t k = 0; k < MM; k++) G[k] = c_add(gi[k], X[k]);
+            }
+            for (int j = 0; j < M; j++) ldos_out[(size_t)i * M + j] = -G[(size_t)j * M + j].im / pi;
+        }
+    }
+    free(gall); free(buf); free(mp);
+    return rc;
+}
+
 /* ==========================================================================================
  * Exported C ABI of the oracle (loaded through ctypes by oracle/rgf_oracle.py).
  * Complex arrays: interleaved doubles, row-major.
@@ -612,4 +673,26 @@ int orc_transmission_brute(int M, int L, const double *onsite, const uint8_t *va
     if (M < 2 || L < 1 || !(eta > 0.0) || !onsite) return ORC_EINVAL;
     if ((long)M * L > 4096) return ORC_EINVAL;
     return brute(M, L, onsite, vac, t, E, eta, lead_method, T_LR, T_RL);
+}
+
+/* ldos_out[n_E][L][M] = -(1/pi) Im G_ii[j][j] of the connected device, OpenMP over energies. */
+int orc_ldos_batch(int M, int L, const double *onsite, const uint8_t *vac, double t, const double *energies, int n_E,
+                   double eta, int lead_method, int nthreads, double *ldos_out)
+{
+    if (M < 2 || L < 1 || n_E < 1 || !(eta > 0.0) || !onsite || !energies || !ldos_out) return ORC_EINVAL;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+    int first = ORC_OK;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int k = 0; k < n_E; k++) {
+        int rc = ldos_sweep(M, L, onsite, vac, t, energies[k], eta, lead_method, ldos_out + (size_t)k * L * M);
+        if (rc != ORC_OK) {
+#pragma omp critical
+            { if (first == ORC_OK) first = rc; }
+        }
+    }
+    return first;
 }

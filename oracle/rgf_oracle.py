@@ -34,6 +34,7 @@ def lib():
         L.orc_transmission.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, dp, dp, ip]
         L.orc_sweep_state.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, dp, dp]
         L.orc_transmission_batch.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, dp, C.c_int, C.c_double, C.c_int, C.c_int, dp, ip]
+        L.orc_ldos_batch.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, dp, C.c_int, C.c_double, C.c_int, C.c_int, dp]
         L.orc_transmission_brute.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, dp, dp]
         _lib = L
     return _lib
@@ -147,3 +148,14 @@ def transmission_brute(onsite, vacancy, t, E, eta, method=LEAD_CELL):
     if rc:
         raise OracleError(rc, "transmission_brute")
     return a.value, b.value
+
+
+def ldos_batch(onsite, vacancy, t, energies, eta, method=LEAD_CELL, nthreads=0):
+    """LDOS[n_E][L][M] = -(1/pi) Im G_ii[j][j] of the connected device (orc_ldos_batch, O9)."""
+    onsite, vac, vp, M, L = _onsite(onsite, vacancy)
+    E = np.ascontiguousarray(energies, dtype=np.float64)
+    out = np.empty((E.shape[0], L, M), dtype=np.float64)
+    rc = lib().orc_ldos_batch(M, L, _dp(onsite), vp, t, _dp(E), E.shape[0], eta, method, nthreads, _dp(out))
+    if rc:
+        raise OracleError(rc, "ldos_batch")
+    return out

@@ -363,3 +363,72 @@ def test_near_neutrality_golden_is_consistent_with_the_oracle(oracle):
         T_or = oracle.transmission_batch(w.onsite[0], vac, w.t, w.energies, w.eta)
         T_ld = np.array([float(r[3]) for r in rows if r[0] == case])
         assert np.all(np.abs(T_or - T_ld) <= 1e-9), (case, np.abs(T_or - T_ld))
+
+
+# ----------------------------------------------------------------------------------------
+# O9: local density of states (diagonal blocks of the connected Green's function), SURVEY.md 8(f) F-4
+# ----------------------------------------------------------------------------------------
+
+def definition_ldos(onsite, vac, t, E, eta, gL, gR):
+    """-(1/pi) Im diag of Eq. 1 written out with numpy: the whole device matrix, inverted at once."""
+    L, M = onsite.shape
+    N = M * L
+    isvac = np.zeros((L, M), dtype=bool) if vac is None else vac.astype(bool)
+    A = (E + 1j * eta) * np.eye(N, dtype=complex)
+    for i in range(L):
+        A[i * M:(i + 1) * M, i * M:(i + 1) * M] -= slice_H(M, onsite[i], t, isvac[i])
+        if i + 1 < L:
+            m = mask(i, M) * (~isvac[i]) * (~isvac[i + 1])
+            A[i * M:(i + 1) * M, (i + 1) * M:(i + 2) * M] -= np.diag(t * m)
+            A[(i + 1) * M:(i + 2) * M, i * M:(i + 1) * M] -= np.diag(t * m)
+    mL = mask(-1, M) * (~isvac[0])
+    mR = mask(L - 1, M) * (~isvac[L - 1])
+    A[:M, :M] -= (t * mL)[:, None] * gL * (t * mL)[None, :]
+    A[N - M:, N - M:] -= (t * mR)[:, None] * gR * (t * mR)[None, :]
+    return (-np.diag(np.linalg.inv(A)).imag / np.pi).reshape(L, M)
+
+
+@pytest.mark.parametrize("M,L", [(4, 1), (5, 2), (6, 7), (9, 6)])
+def test_ldos_recursion_equals_definition(oracle, M, L):
+    """The two-pass recursion against the full inverse, with disorder, vacancies (incl. both end slices), odd M and L."""
+    on = inputs.anderson(M, L, 0.4, 50 + M)
+    vac = np.zeros((L, M), dtype=np.uint8)
+    vac[0, 1] = 1
+    if L > 2:
+        vac[L // 2, 0] = vac[L - 1, M - 2] = 1
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.array([-1.7, -0.3, 0.45, 1.2])
+    for eta in (1e-3, 1e-6):
+        got = oracle.ldos_batch(on, vac, T_HOP, E, eta)
+        for k, e in enumerate(E):
+            gL, _ = oracle.lead_surface(M, L, T_HOP, e, eta, -1)
+            gR, _ = oracle.lead_surface(M, L, T_HOP, e, eta, +1)
+            ref = definition_ldos(on, vac, T_HOP, e, eta, gL, gR)
+            assert np.max(np.abs(got[k] - ref)) <= 1e-10 * max(1.0, np.max(np.abs(ref))), (M, L, e, eta)
+
+
+def test_ldos_closed_forms_and_invariants(oracle):
+    M, L, eta = 8, 6, 1e-3
+    E = np.array([-0.9, 0.37])
+    # a vacancy is an isolated level at its on-site energy: G = 1 / (z - eps), LDOS = (eta / pi) / ((E - eps)^2 + eta^2)
+    on = np.zeros((L, M))
+    vac = np.zeros((L, M), dtype=np.uint8)
+    vac[2, 3] = 1
+    on[2, 3] = 0.5
+    got = oracle.ldos_batch(on, vac, T_HOP, E, eta)
+    for k, e in enumerate(E):
+        assert abs(got[k, 2, 3] - (eta / np.pi) / ((e - 0.5) ** 2 + eta ** 2)) < 1e-12
+    # clean ribbon between clean leads = infinite ribbon: LDOS >= 0, periodic with the two-slice cell, and (zero on-site
+    # energies, bipartite lattice) the same at E and -E
+    clean = oracle.ldos_batch(np.zeros((L, M)), None, T_HOP, np.array([0.8, -0.8, 1.9]), eta)
+    assert np.all(clean > 0)
+    assert np.max(np.abs(clean[:, 2:] - clean[:, :-2])) < 1e-9 * np.max(clean)
+    assert np.max(np.abs(clean[0] - clean[1])) < 1e-12 * np.max(clean)
+    # one-dimensional check of the scale: M = 2 ... the integrated weight of a site is 1 (Lorentzian tails of width eta):
+    # a single isolated device site (both neighbours vacant) integrates to 1
+    on1 = np.zeros((3, 3))
+    v1 = np.ones((3, 3), dtype=np.uint8)
+    v1[1, 1] = 0                       # only the centre site is not a vacancy; every bond to it is cut
+    grid = np.linspace(-0.2, 0.2, 4001)
+    w = oracle.ldos_batch(on1, v1, T_HOP, grid, 5e-3)[:, 1, 1]
+    assert abs(np.trapezoid(w, grid) - 2 / np.pi * np.arctan(0.2 / 5e-3)) < 1e-6
