@@ -55,6 +55,7 @@ def parse():
     ap.add_argument("--cohort", type=int, default=0)
     ap.add_argument("--form", default="half", choices=["half", "dense"], help="formulation of the sweep (include/rgf.h)")
     ap.add_argument("--no-guard", action="store_true", help="switch the near-neutrality guard off (rgf_set_guard 0)")
+    ap.add_argument("--ldos", action="store_true", help="time the second workload instead (rgf_ldos, SURVEY.md 8(f) F-4): M, L as given, n-E energies")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -179,10 +180,42 @@ def run_reference(a):
     print(json.dumps(line))
 
 
+def run_ldos(a):
+    """Second workload (not the headline line): LDOS of the connected device, three batched M x M inverses per slice."""
+    import torch
+    from paper_1107_5300_b200 import binding as rgf
+    w = inputs.config2(M=a.M, L=a.L, n_E=a.n_E)
+    plan = rgf.rgf_plan_create(0, torch.cuda.current_stream().cuda_stream)
+    peak = rgf.rgf_fp64_peak_tflops(plan)
+    rgf.rgf_set_device(plan, w.M, w.L, np.ascontiguousarray(w.onsite[0]), w.t, None)
+    E = torch.from_numpy(w.energies).cuda()
+    out = torch.empty((1, w.n_E, w.L, w.M), dtype=torch.float64, device="cuda")
+    eta = 2.0 / w.n_E
+    for _ in range(max(1, a.warmup)):
+        rgf.rgf_ldos(plan, E, w.n_E, eta, out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(a.steps):
+        rgf.rgf_ldos(plan, E, w.n_E, eta, out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / a.steps
+    st = rgf.rgf_get_stats(plan)
+    flops = 3 * 8.0 * w.M ** 3 * w.n_E * w.L
+    print(json.dumps({"metric": "rgf_ldos_slice_steps_per_s", "value": w.n_E * w.L / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": a.steps,
+                      "config": {"workload": "LDOS of the configs[2] ribbon, M=%d L=%d n_E=%d, eta=%.3g eV, complex128" % (w.M, w.L, w.n_E, eta), "chunk": st["cohort"]},
+                      "tflops_executed": flops / (ms * 1e-3) * 1e-12, "frac_of_fp64_tensor_peak": flops / (ms * 1e-3) * 1e-12 / peak, "peak": peak,
+                      "gpu_launches": st["launches"], "dtype": "f64", "data": "synthetic"}))
+    rgf.rgf_destroy(plan)
+
+
 def main():
     a = parse()
     if a.impl == "reference":
         return run_reference(a)
+    if a.ldos:
+        return run_ldos(a)
     import torch
     from paper_1107_5300_b200 import binding as rgf     # fails loudly if the CUDA library is missing
 

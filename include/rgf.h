@@ -183,6 +183,17 @@ int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, 
 int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int precision,
                     int nslices, double *g_out, double *P_out);
 
+/* ---- second workload on the same kernels ---------------------------------------------------------
+ * Local density of states of the device connected to both leads ("any desired quantity, e.g. charge density";
+ * the Green's functions of the whole region):
+ *     ldos_out[n_dev][n_E][L][M] = -(1/pi) Im G_ii[j][j],   G = (z - H_device - Sigma_L (+) 0 (+) Sigma_R)^-1  (Eq. 1)
+ * by the recursion applied from both ends (three batched M x M inverses per slice; only the (M/2)-blocks the inter-slice
+ * coupling keeps are stored between the two passes, in chunks of matrices that fit half of the free device memory).
+ * The charge density is the caller's energy integral of it.  energies / ldos_out: host or device pointers; complex128;
+ * eta as in rgf_transmission (an LDOS on a grid wants eta of the order of the grid spacing).  A matrix that hits a zero /
+ * non-finite pivot has NaN from that slice on and RGF_ESINGULAR is returned. */
+int rgf_ldos(rgf_plan *p, const double *energies, int n_E, double eta, double *ldos_out);
+
 /* ---- allocation-free entry point --------------------------------------------------------------------------
  * A4 alone like rgf_inverse_batched (same kernels, n <= 256 path), for callers that cannot call cudaMalloc: code under CUDA
  * graph capture, tight serving loops, harnesses that forbid allocation.  It takes no plan and calls no cudaMalloc, cudaFree

@@ -49,6 +49,7 @@ _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
 _lib.rgf_sweep_state.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, C.c_int, _vp, _vp]
+_lib.rgf_ldos.argtypes = [_vp, _vp, C.c_int, C.c_double, _vp]
 _lib.rgf_inverse_batched_static.argtypes = [C.c_int, _vp, C.c_int, C.c_int, _vp, _vp, _vp]
 _lib.rgf_static_last_error.restype = C.c_char_p
 
@@ -158,6 +159,10 @@ def rgf_sweep_state(plan, dev, energies, n_E, eta, precision, nslices, g_out, P_
     return _check(plan, _lib.rgf_sweep_state(plan, dev, _addr(energies), n_E, eta, precision, nslices, _addr(g_out), _addr(P_out)))
 
 
+def rgf_ldos(plan, energies, n_E, eta, ldos_out):
+    return _check(plan, _lib.rgf_ldos(plan, _addr(energies), n_E, eta, _addr(ldos_out)))
+
+
 def rgf_static_last_error():
     return _lib.rgf_static_last_error().decode()
 
@@ -203,6 +208,13 @@ class Plan:
         T = np.empty((self.n_dev, energies.shape[0]), dtype=np.float64)
         rgf_transmission(self.handle, energies, energies.shape[0], eta, precision, T, ok)
         return T
+
+    def ldos(self, energies, eta):
+        """Host convenience: numpy energies in, numpy LDOS[n_dev][n_E][L][M] out."""
+        energies = np.ascontiguousarray(energies, dtype=np.float64)
+        out = np.empty((self.n_dev, energies.shape[0], self.L, self.M), dtype=np.float64)
+        rgf_ldos(self.handle, energies, energies.shape[0], eta, out)
+        return out
 
     def stats(self):
         return rgf_get_stats(self.handle)

@@ -25,6 +25,7 @@
 #include "half_sweep.cuh"
 #include "half_sweep_c64.cuh"
 #include "lead_modes.cuh"
+#include "ldos_kernels.cuh"
 #include "rgf_common.cuh"
 #include "sweep_kernels.cuh"
 #include "zgemm.cuh"
@@ -69,6 +70,7 @@ struct rgf_plan {
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
     Buf lc_S3, lc_R;                              // run_lead_side_schur: S again and the residual of its inverse
+    Buf ld_A0, ld_A1, ld_B0, ld_B1, ld_stash, ld_out;   // rgf_ldos: two inverse ping-pong pairs, the stashed gR blocks, the LDOS of a chunk
     Buf lm_Q;                                     // mode-space leads: the orthogonal basis Q [nc][nc]
     Buf lead_status;                              // [n_E] bad pivot inside the lead decimation of an energy
     int lead_method = RGF_LEAD_MODE_SPACE;
@@ -1021,7 +1023,7 @@ int rgf_destroy(rgf_plan *p)
     if (p->stream) cudaStreamSynchronize(p->stream);
     Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->pivmin, &p->gsq, &p->T_keep, &p->redo_idx,
                    &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3,
-                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status};
+                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status, &p->ld_A0, &p->ld_A1, &p->ld_B0, &p->ld_B1, &p->ld_stash, &p->ld_out};
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
@@ -1230,6 +1232,90 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     CUDA_TRY(p, cudaMemcpyAsync(P_out, p->stage_out.p, bytes, cudaMemcpyDefault, p->stream));
     CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     drain_update_events(p);
+    return RGF_OK;
+}
+
+// F-4: local density of states of the connected device, LDOS[n_dev][n_E][L][M] (ldos_kernels.cuh states the recursion).
+// Three batched M x M inverses per slice and matrix (gR_i on the way back, gL_i and G_ii on the way forth); the gR blocks
+// of a chunk of matrices are stashed in HBM between the two passes, the chunk sized to at most half of the free memory.
+int rgf_ldos(rgf_plan *p, const double *energies, int n_E, double eta, double *ldos_out)
+{
+    int rc = begin_call(p);
+    if (rc) return rc;
+    if (!p->has_device) return fail(p, RGF_ESTATE, "rgf_ldos before rgf_set_device");
+    if (!ldos_out) return fail(p, RGF_EINVAL, "ldos_out is NULL");
+    if (n_E >= 1 && (long long)p->n_dev * n_E > 65535)
+        return fail(p, RGF_EUNSUPPORTED, "n_dev * n_E = %lld > 65535 batch items per call: split the energy grid", (long long)p->n_dev * n_E);
+    memset(&p->stats, 0, sizeof(p->stats));
+    CUDA_TRY(p, cudaEventRecord(p->ev[0], p->stream));
+    if ((rc = upload_energies(p, energies, n_E, eta))) return rc;
+    const int M = p->M, L = p->L, nh = p->nh, batch = p->n_dev * n_E;
+    const size_t MM = (size_t)M * M;
+    if ((rc = ensure(p, p->status, sizeof(int) * (size_t)batch))) return rc;
+    CUDA_TRY(p, cudaMemsetAsync(p->status.p, 0, sizeof(int) * (size_t)batch, p->stream));
+    int lead_open = 0;
+    if ((rc = run_leads(p, n_E, eta, &lead_open))) return rc;
+    if (lead_open) return fail(p, RGF_ENOCONV, "lead decimation did not converge for %d energies", lead_open);
+    // chunk of matrices whose stash fits
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(p, cudaMemGetInfo(&free_b, &total_b));
+    const size_t per_matrix = sizeof(cplx) * ((size_t)L * nh * nh + 4 * MM + (size_t)n_E * 0) + sizeof(double) * (size_t)L * M + sizeof(cplx) * (size_t)M * 64;
+    size_t have = free_b / 2 + p->ld_stash.cap + p->ld_out.cap;
+    int chunk = (int)std::min<size_t>((size_t)batch, std::max<size_t>(1, have / per_matrix));
+    Ws &w = p->ws[0];
+    Buf *four[] = {&p->ld_A0, &p->ld_A1, &p->ld_B0, &p->ld_B1};
+    for (Buf *b : four) if ((rc = ensure(p, *b, sizeof(cplx) * MM * chunk))) return rc;
+    if ((rc = ensure(p, p->ld_stash, sizeof(cplx) * (size_t)L * nh * nh * chunk))) return rc;
+    if ((rc = ensure(p, p->ld_out, sizeof(double) * (size_t)L * M * chunk))) return rc;
+    if ((rc = ensure_inverse_ws(p, w, M, chunk))) return rc;
+    p->stats.cohort = chunk;
+    const double *E = ptr<double>(p->E);
+    const cplx *gLl = ptr<cplx>(p->gL), *gRl = lead_gR(p);
+    cplx *stash = ptr<cplx>(p->ld_stash);
+    for (int bz0 = 0; bz0 < batch; bz0 += chunk) {
+        const int nb = std::min(chunk, batch - bz0);
+        int *status = ptr<int>(p->status) + bz0;
+        dim3 ag((unsigned)std::min<size_t>((MM + 255) / 256, 2048), nb), sg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
+        const size_t sslice = (size_t)nh * nh * nb;          // stash of one slice for the chunk
+        auto assemble = [&](cplx *A, int i, bool left, const cplx *gprev, bool right) {
+            ldos_assemble_kernel<<<ag, 256, 0, p->stream>>>(A, M, L, nh, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                           ptr<uint8_t>(p->hop), left ? 1 : 0, gprev, gLl, right ? 1 : 0,
+                                                           i + 1 < L ? stash + (size_t)(i + 1) * sslice : nullptr, gRl);
+            p->stats.launches++;
+        };
+        cplx *A0 = ptr<cplx>(p->ld_A0), *A1 = ptr<cplx>(p->ld_A1), *P = ptr<cplx>(p->ld_B0), *Q = ptr<cplx>(p->ld_B1), *res = nullptr;
+        // right-to-left: gR_i, i = L-1 .. 1; slice i - 1 needs its block on S_{i-1}
+        for (int i = L - 1; i >= 1; i--) {
+            assemble(A0, i, false, nullptr, true);
+            if ((rc = run_inverse(p, w, A0, A1, M, nb, status, &res))) return rc;
+            ldos_stash_kernel<<<sg, 256, 0, p->stream>>>(res, stash + (size_t)i * sslice, M, nh, (i - 1) & 1);
+            p->stats.launches++;
+        }
+        // left-to-right: G_ii and gL_i
+        for (int i = 0; i < L; i++) {
+            assemble(A0, i, true, P, true);
+            if (i + 1 < L) assemble(Q, i, true, P, false);
+            if ((rc = run_inverse(p, w, A0, A1, M, nb, status, &res))) return rc;
+            ldos_diag_kernel<<<(nb * M + 255) / 256, 256, 0, p->stream>>>(res, ptr<double>(p->ld_out), status, M, L, i, nb);
+            p->stats.launches++;
+            if (i + 1 < L) {
+                if ((rc = run_inverse(p, w, Q, P, M, nb, status, &res))) return rc;
+                if (res != P) std::swap(P, Q);            // P = gL_i for the next slice
+            }
+        }
+        CUDA_TRY(p, cudaGetLastError());
+        CUDA_TRY(p, cudaMemcpyAsync(ldos_out + (size_t)bz0 * L * M, p->ld_out.p, sizeof(double) * (size_t)L * M * nb, cudaMemcpyDefault, p->stream));
+        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    }
+    CUDA_TRY(p, cudaEventRecord(p->ev[4], p->stream));
+    std::vector<int> h_status(batch);
+    CUDA_TRY(p, cudaMemcpyAsync(h_status.data(), p->status.p, sizeof(int) * (size_t)batch, cudaMemcpyDeviceToHost, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    drain_update_events(p);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, p->ev[0], p->ev[4]); p->stats.ms_total = ms; p->stats.ms_sweep = ms;
+    for (int b = 0; b < batch; b++)
+        if (h_status[b]) return fail(p, RGF_ESINGULAR, "zero or non-finite pivot (first at batch item %d); its LDOS is NaN from that slice on", b);
     return RGF_OK;
 }
 

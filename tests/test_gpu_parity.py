@@ -433,3 +433,41 @@ def test_guard_indicator_tracks_the_resonance(rgf, plan):
     print("guard indicators", G, Gmax)
     assert G[0] < 50 and np.all(G[1:] > 0.2 * 2.7 / E[1:]) and np.all(G[1:] < 20 * 2.7 / E[1:])
     assert np.all(Gmax >= G * 0.99) and np.all(Gmax < 2.0 * G + 50)      # clean ribbon: every half-step has the same pivot
+
+
+# ---- F-4: local density of states of the connected device (rgf_ldos) ---------------------------------------------------------
+
+@pytest.mark.parametrize("M,L,W,with_vac", [(20, 12, 0.25, False), (21, 9, 0.3, True), (64, 10, 0.1, True), (20, 1, 0.2, False),
+                                             (128, 7, 0.25, False), (300, 3, 0.1, True)])
+def test_ldos_matches_oracle(rgf, plan, oracle, M, L, W, with_vac):
+    """LDOS[i][j] = -(1/pi) Im G_ii[j][j] element by element against the oracle's two-pass recursion (itself pinned to the full
+    inverse); two devices batched, eta = 1e-3 eV (a smooth LDOS).  Tolerance 1e-9 max(1, max LDOS)."""
+    on = np.stack([inputs.anderson(M, L, W, 300 + M), inputs.anderson(M, L, W, 301 + M)])
+    vac = None
+    if with_vac:
+        vac = np.zeros((2, L, M), dtype=np.uint8)
+        vac[0, 0, 1] = vac[0, L - 1, 2] = vac[1, L // 2, 0] = 1
+        on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.array([-1.3, -0.2, 0.07, 0.9, 2.1])
+    plan.set_device(on, -2.7, vac)
+    got = plan.ldos(E, 1e-3)
+    assert got.shape == (2, len(E), L, M)
+    for d in range(2):
+        ref = oracle.ldos_batch(on[d], None if vac is None else vac[d], -2.7, E, 1e-3)
+        err = np.max(np.abs(got[d] - ref))
+        assert err <= 1e-9 * max(1.0, np.max(np.abs(ref))), (M, L, d, err, np.max(np.abs(ref)))
+    assert np.all(got > 0)
+    assert plan.stats()["launches"] > 0
+
+
+def test_ldos_device_pointers_and_chunks(rgf, plan, oracle):
+    import torch
+    M, L = 32, 8
+    on = inputs.anderson(M, L, 0.2, 9)
+    plan.set_device(on, -2.7)
+    E = np.linspace(-1.0, 1.0, 6)
+    E_dev = torch.tensor(E, dtype=torch.float64, device="cuda")
+    out = torch.empty((1, 6, L, M), dtype=torch.float64, device="cuda")
+    rgf.rgf_ldos(plan.handle, E_dev, 6, 2e-3, out)
+    ref = oracle.ldos_batch(on, None, -2.7, E, 2e-3)
+    assert np.max(np.abs(out.cpu().numpy()[0] - ref)) <= 1e-9 * max(1.0, np.max(ref))
