@@ -63,8 +63,10 @@ def parse():
 
 def workload(a, world, rank):
     """Headline ribbon; with N GPUs the global grid has 512*N energies and rank r takes E[r::N] (weak scaling)."""
+    from paper_1107_5300_b200 import binding as rgf
     w = inputs.config2(M=a.M, L=a.L, n_E=a.n_E * world)
-    E = np.ascontiguousarray(w.energies[rank::world])
+    E = np.empty(rgf.rgf_shard_count(w.n_E, world, rank))
+    rgf.rgf_shard_energies(w.energies, w.n_E, world, rank, E)          # the library's round-robin split (include/rgf.h)
     return w, E
 
 

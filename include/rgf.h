@@ -183,6 +183,17 @@ int rgf_lead_self_energy(rgf_plan *p, int dev, const double *energies, int n_E, 
 int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, double eta, int precision,
                     int nslices, double *g_out, double *P_out);
 
+/* ---- multi-GPU convention (the path shards over energies, nothing is exchanged) -------------------------
+ * One process per GPU, each with its own plan; rank r of `world` computes energies[r], energies[r + world], ... (round-robin:
+ * the cost per energy is uniform but failures and guard redos cluster near charge neutrality).  HOST pointers only.
+ *   rgf_shard_count     number of energies of rank `rank` (or RGF_EINVAL)
+ *   rgf_shard_energies  writes them to shard_out[count]; returns count
+ *   rgf_unshard         scatters a rank's result T_shard[n_dev][count] into its places of T_full[n_dev][n_E]; after every
+ *                       rank's part has been scattered (e.g. from an all-gather) T_full is the single-GPU result. */
+int rgf_shard_count(int n_E, int world, int rank);
+int rgf_shard_energies(const double *energies, int n_E, int world, int rank, double *shard_out);
+int rgf_unshard(const double *T_shard, int n_dev, int n_E, int world, int rank, double *T_full);
+
 /* ---- second workload on the same kernels ---------------------------------------------------------
  * Local density of states of the device connected to both leads ("any desired quantity, e.g. charge density";
  * the Green's functions of the whole region):

@@ -49,6 +49,9 @@ _lib.rgf_fp64_peak_tflops.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rgf_inverse_batched.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
 _lib.rgf_lead_self_energy.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, _vp, C.POINTER(C.c_int)]
 _lib.rgf_sweep_state.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_double, C.c_int, C.c_int, _vp, _vp]
+_lib.rgf_shard_count.argtypes = [C.c_int, C.c_int, C.c_int]
+_lib.rgf_shard_energies.argtypes = [_vp, C.c_int, C.c_int, C.c_int, _vp]
+_lib.rgf_unshard.argtypes = [_vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp]
 _lib.rgf_ldos.argtypes = [_vp, _vp, C.c_int, C.c_double, _vp]
 _lib.rgf_inverse_batched_static.argtypes = [C.c_int, _vp, C.c_int, C.c_int, _vp, _vp, _vp]
 _lib.rgf_static_last_error.restype = C.c_char_p
@@ -157,6 +160,22 @@ def rgf_lead_self_energy(plan, dev, energies, n_E, eta, side, Sigma_out):
 
 def rgf_sweep_state(plan, dev, energies, n_E, eta, precision, nslices, g_out, P_out):
     return _check(plan, _lib.rgf_sweep_state(plan, dev, _addr(energies), n_E, eta, precision, nslices, _addr(g_out), _addr(P_out)))
+
+
+def rgf_shard_count(n_E, world, rank):
+    return _lib.rgf_shard_count(n_E, world, rank)
+
+
+def rgf_shard_energies(energies, n_E, world, rank, shard_out):
+    """Host numpy arrays; returns the number of energies written."""
+    return _lib.rgf_shard_energies(_addr(energies, np.float64), n_E, world, rank, _addr(shard_out, np.float64))
+
+
+def rgf_unshard(T_shard, n_dev, n_E, world, rank, T_full):
+    rc = _lib.rgf_unshard(_addr(T_shard, np.float64), n_dev, n_E, world, rank, _addr(T_full, np.float64))
+    if rc != RGF_OK:
+        raise RgfError(rc, "rgf_unshard: bad argument")
+    return rc
 
 
 def rgf_ldos(plan, energies, n_E, eta, ldos_out):

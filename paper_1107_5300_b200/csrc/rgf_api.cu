@@ -1235,6 +1235,31 @@ int rgf_sweep_state(rgf_plan *p, int dev, const double *energies, int n_E, doubl
     return RGF_OK;
 }
 
+// ---- multi-GPU convention: (seed, energy) pairs are independent, so N ranks split the energy grid
+// round-robin, rank r taking energies[r], energies[r + N], ...; no data-path collective.  Host-only helpers, no CUDA call.
+int rgf_shard_count(int n_E, int world, int rank)
+{
+    if (n_E < 0 || world < 1 || rank < 0 || rank >= world) return RGF_EINVAL;
+    return n_E > rank ? (n_E - rank + world - 1) / world : 0;
+}
+
+int rgf_shard_energies(const double *energies, int n_E, int world, int rank, double *shard_out)
+{
+    const int cnt = rgf_shard_count(n_E, world, rank);
+    if (cnt < 0 || !energies || !shard_out) return RGF_EINVAL;
+    for (int k = 0; k < cnt; k++) shard_out[k] = energies[rank + (long long)k * world];
+    return cnt;
+}
+
+int rgf_unshard(const double *T_shard, int n_dev, int n_E, int world, int rank, double *T_full)
+{
+    const int cnt = rgf_shard_count(n_E, world, rank);
+    if (cnt < 0 || n_dev < 1 || !T_shard || !T_full) return RGF_EINVAL;
+    for (int d = 0; d < n_dev; d++)
+        for (int k = 0; k < cnt; k++) T_full[(long long)d * n_E + rank + (long long)k * world] = T_shard[(long long)d * cnt + k];
+    return RGF_OK;
+}
+
 // F-4: local density of states of the connected device, LDOS[n_dev][n_E][L][M] (ldos_kernels.cuh states the recursion).
 // Three batched M x M inverses per slice and matrix (gR_i on the way back, gL_i and G_ii on the way forth); the gR blocks
 // of a chunk of matrices are stashed in HBM between the two passes, the chunk sized to at most half of the free memory.

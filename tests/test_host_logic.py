@@ -64,6 +64,25 @@ def test_shard_roundtrip():
         assert np.array_equal(inputs.unshard(parts, 13), E)
 
 
+def test_library_shard_helpers_match_the_generator_side():
+    """rgf_shard_count / rgf_shard_energies / rgf_unshard (host-only C ABI) against numpy slicing, ragged counts included."""
+    from paper_1107_5300_b200 import binding as rgf, inputs
+    E = np.linspace(-1, 1, 13)
+    for world in (1, 2, 3, 5, 8, 16):
+        full = np.full((2, 13), np.nan)
+        for r in range(world):
+            cnt = rgf.rgf_shard_count(13, world, r)
+            assert cnt == len(inputs.shard(E, world, r))
+            mine = np.empty(max(cnt, 1))
+            assert rgf.rgf_shard_energies(E, 13, world, r, mine) == cnt
+            assert np.array_equal(mine[:cnt], inputs.shard(E, world, r))
+            part = np.ascontiguousarray(np.stack([mine[:cnt] * 10, mine[:cnt] * 100]))
+            if cnt:
+                rgf.rgf_unshard(part, 2, 13, world, r, full)
+        assert np.array_equal(full, np.stack([E * 10, E * 100]))
+    assert rgf.rgf_shard_count(13, 2, 2) == rgf.RGF_EINVAL and rgf.rgf_shard_count(13, 0, 0) == rgf.RGF_EINVAL
+
+
 _WORKER = r"""
 import os, sys
 import numpy as np
