@@ -4,15 +4,16 @@
 //
 // One panel step k (columns K = [k0, k0+32)), for every matrix of the batch:
 //   gj32_panel_kernel : reads X[:, K]; Gauss-Jordan with partial pivoting on the n x 32 panel held
-//                       in shared memory (4 sub-blocks of 8 columns: rank-1 DFMA updates inside the
-//                       sub-block with the thread's row in registers, then one (n x 8) x (8 x 24)
-//                       DMMA product for the other panel columns).  Rows are never moved; the
+//                       in shared memory, by hs_factor_panel of half_sweep.cuh (4 sub-blocks of 8 columns:
+//                       pivot steps with the thread's row in registers, then one (n x 8) x (8 x 24) DMMA
+//                       product for the other panel columns).  Rows are never moved; the
 //                       exchange is the map rowAt[pos] = row of X that belongs at position pos.
 //                       Writes Y[pos, K] = N'[rowAt[pos], :], Mult[pos, :] = N' - E, rowAt, orig.
 //   gj32_update_kernel: Y[pos, J] = X[rowAt[pos], J] + Mult[pos, :] * X[rowAt[k0 + :], J]   (FP64 DMMA)
 // then X <-> Y.  After the last panel gj32_unpermute_kernel scatters columns: out[:, orig[pos]] = X[:, pos].
 // (Eq. 4 / PAPER.md:53 "one call of the linear equation solver".)
 #pragma once
+#include "half_sweep.cuh"
 #include "rgf_common.cuh"
 
 namespace rgf {
@@ -23,24 +24,28 @@ constexpr int G32_LDR = G32_B + 2;      // 34
 __host__ __device__ constexpr size_t gj32_panel_smem(int n)
 {
     return sizeof(cplx) * ((size_t)G32_NT * G32_LDP + G32_SB * G32_LDR + 2 * (G32_NT / 32) * (G32_SB + 1)) + sizeof(unsigned) * 4 * (G32_NT / 32) +
-           sizeof(int) * (2 * (size_t)n + G32_B + 8) + 64;
+           sizeof(int) * (4 * (size_t)n + G32_B + 8) + 64;
 }
 
+// The factorisation itself is hs_factor_panel of half_sweep.cuh (one implementation of the pivot step and of the in-panel
+// DMMA update for the fused kernel and for this one): thread = row, all eight warps search and update.
 __global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restrict__ Xall, cplx *__restrict__ Yall, long long g_batch,
                                                             int n, int k0, cplx *__restrict__ Mall, int *__restrict__ rowAtAll,
                                                             int *__restrict__ origall, int *__restrict__ status)
 {
     constexpr int B = G32_B, SB = G32_SB, NT = G32_NT, LDP = G32_LDP, LDR = G32_LDR;
+    static_assert(G32_B == HS_B && G32_SB == HS_SB && G32_LDP == HS_LDP && G32_LDR == HS_LDR && G32_NT == HS_NT, "shares hs_factor_panel");
     extern __shared__ __align__(16) unsigned char gj_smem[];
     cplx *panel = reinterpret_cast<cplx *>(gj_smem);           // [NT][LDP], rows in X order
     cplx *Rs = panel + NT * LDP;                                // [SB][LDR] pivot rows of the sub-block
     cplx *crow = Rs + SB * LDR;                                 // [2][NT/32][SB] candidate pivot rows
     cplx *cinv = crow + 2 * (NT / 32) * SB;                     // [2][NT/32] 1 / candidate pivot
-    unsigned *ckey = reinterpret_cast<unsigned *>(cinv + 2 * (NT / 32));               // [2][NT/32]
-    int *cidx = reinterpret_cast<int *>(ckey + 2 * (NT / 32));                         // [2][NT/32]
-    int *rowAt = cidx + 2 * (NT / 32);
+    unsigned *ckey = reinterpret_cast<unsigned *>(cinv + 2 * (NT / 32));               // [2][NT/32], 16-byte aligned
+    unsigned *pivmin = ckey + 2 * (NT / 32);                                           // [1] (+ padding to 2 * NT / 32)
+    int *rowAt = reinterpret_cast<int *>(pivmin + 2 * (NT / 32));
     int *posOf = rowAt + n;
-    int *prow = posOf + n;                                      // [B]
+    int *perm = posOf + n, *pinv = perm + n;                    // scratch of hs_factor_panel (pivot row of a column and back)
+    int *prow = pinv + n;                                       // [B]
 
     const int b = blockIdx.x;
     const cplx *X = Xall + (long long)b * g_batch;
@@ -48,7 +53,7 @@ __global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restri
     cplx *Mult = Mall + (long long)b * n * B;
     int *orig = origall + (long long)b * n;
     int *rowAtG = rowAtAll + (long long)b * n;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const int tid = threadIdx.x, warp = tid >> 5;
     const int r = tid;
     const bool has_row = r < n;
     const int bw = (n - k0 < B) ? (n - k0) : B;
@@ -65,119 +70,28 @@ __global__ void __launch_bounds__(G32_NT) gj32_panel_kernel(const cplx *__restri
     cp_async_wait<0>();
     __syncthreads();
 
-    for (int s = 0; s < B / SB; s++) {
-        const int c0 = s * SB;
-        const int ncols = bw - c0 < SB ? bw - c0 : SB;
-        if (ncols <= 0) break;
-        cplx row[SB];
-#pragma unroll
-        for (int j = 0; j < SB; j++) row[j] = panel[r * LDP + c0 + j];
-#pragma unroll 1
-        for (int cc = 0; cc < ncols; cc++) {
-            const int pb = (cc & 1) * (NT / 32);           // candidate buffers alternate: one barrier per column
-            cplx x = row[0];
-#pragma unroll
-            for (int j = 1; j < SB; j++) if (j == cc) x = row[j];
-            // ---- pivot search.  32-bit key = top 24 bits of |x|^2 (sign, exponent, 12 mantissa bits) and
-            // 255 - warp: the block maximum is a pivot within 2^-12 of the largest magnitude (any such
-            // pivot is as good as the exact maximum), lowest warp / lowest lane on ties.  Each warp's
-            // candidate lane publishes its raw row, its row index and 1/x, so one barrier per column suffices.
-            const double v = cabs2(x);
-            unsigned hi = used ? 0u : ((unsigned)__double2hiint(v) & 0xffffff00u);
-            if (!used && !(v == v)) hi = 0x7ff80000u;                 // NaN: report it
-            const unsigned wmax = __reduce_max_sync(0xffffffffu, hi);
-            const unsigned ball = __ballot_sync(0xffffffffu, hi == wmax);
-            if (lane == __ffs(ball) - 1) {
-                ckey[pb + warp] = wmax | (unsigned)(255 - warp);
-                cidx[pb + warp] = r;
-                const double iv = 1.0 / v;                             // 1/x = conj(x) / |x|^2
-                cinv[pb + warp] = cmake(x.x * iv, -x.y * iv);
-#pragma unroll
-                for (int j = 0; j < SB; j++) crow[(pb + warp) * SB + j] = row[j];
-            }
-            __syncthreads();
-            unsigned best = ckey[pb];
-#pragma unroll
-            for (int w = 1; w < NT / 32; w++) best = max(best, ckey[pb + w]);
-            const int pw = 255 - (int)(best & 0xffu);
-            const int pr = cidx[pb + pw];
-            const cplx d = cinv[pb + pw];
-            if (r == pr) {
-                if ((best >> 8) == 0u || best >= 0x7ff00000u) status[b] = 1;     // zero / non-finite pivot
-#pragma unroll
-                for (int j = 0; j < SB; j++) row[j] = (j == cc) ? d : cmul(row[j], d);
-                used = true;
-                const int k = k0 + c0 + cc, a = rowAt[k], pp = posOf[pr];
-                rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
-                prow[c0 + cc] = pr;
-            } else {
-                // row -= (x / x_piv) * pivot row; the pivot column itself becomes -x / x_piv
-                const cplx f = cmul(x, d);
-#pragma unroll
-                for (int j = 0; j < SB; j++) {
-                    const cplx pj = crow[(pb + pw) * SB + j];
-                    cplx y = row[j];
-                    cfnma(y, f, pj);
-                    row[j] = (j == cc) ? cmake(-f.x, -f.y) : y;
-                }
-            }
+    HSView v;
+    v.panel = panel; v.Rs = Rs; v.crow = crow; v.cinv = cinv; v.ckey = ckey; v.prow = prow; v.perm = perm; v.pinv = pinv; v.pivmin = pivmin;
+    HSGroup g;
+    g.r = tid; g.slot = warp; g.nslots = (n + 31) >> 5; g.gtid = tid; g.gnt = NT;
+    g.bar_pivot = 1; g.n_pivot = g.nslots * 32; g.bar_all = 0;
+    g.rbase = warp * 32; g.nbsel = 0; g.nbmod = 1;
+    hs_factor_panel<SB>(v, g, n, k0, bw, used, status + b);
+    // the exchanges, in pivot order: position k0 + c takes row prow[c]
+    if (tid == 0)
+        for (int c = 0; c < bw; c++) {
+            const int k = k0 + c, pr = prow[c], a = rowAt[k], pp = posOf[pr];
+            rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
         }
-        __syncthreads();
-        // ---- N'_s back to the panel; snapshot of the sub-block's pivot rows (their other columns)
-#pragma unroll
-        for (int j = 0; j < SB; j++) panel[r * LDP + c0 + j] = row[j];
-        for (int e = tid; e < SB * B; e += NT) {
-            int k = e / B, c = e % B;
-            if (c < c0 || c >= c0 + SB) Rs[k * LDR + c] = (k < ncols) ? panel[prow[c0 + k] * LDP + c] : cmake(0.0, 0.0);
-        }
-        __syncthreads();
-        // ---- other panel columns: panel[:, J] += (N'_s - E_s) (n x 8) * Rs[:, J] (8 x |J|) on DMMA
-        const int nbmax = (bw + 7) / 8;
-        if (nbmax > 1) {
-            int pk[2];
-#pragma unroll
-            for (int q = 0; q < 2; q++) pk[q] = (q * 4 + t < ncols) ? prow[c0 + q * 4 + t] : -1;
-            cplx a[2][4];
-#pragma unroll
-            for (int q = 0; q < 2; q++)
-#pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    const int rr = warp * 32 + i * 8 + g;
-                    a[q][i] = panel[rr * LDP + c0 + q * 4 + t];
-                    if (rr == pk[q]) a[q][i].x -= 1.0;
-                }
-            for (int nb = 0; nb < nbmax; nb++) {
-                if (nb == s) continue;
-                double cre[4][2], cim[4][2];
-                cplx *Cw = panel + (warp * 32) * LDP + nb * 8;
-#pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    cplx v0 = Cw[(i * 8 + g) * LDP + 2 * t], v1 = Cw[(i * 8 + g) * LDP + 2 * t + 1];
-                    cre[i][0] = v0.x; cim[i][0] = v0.y; cre[i][1] = v1.x; cim[i][1] = v1.y;
-                }
-#pragma unroll
-                for (int q = 0; q < 2; q++) {
-                    cplx bb = Rs[(q * 4 + t) * LDR + nb * 8 + g];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) zmma884(cre[i], cim[i], a[q][i].x, a[q][i].y, -a[q][i].y, bb.x, bb.y);
-                }
-#pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    Cw[(i * 8 + g) * LDP + 2 * t] = cmake(cre[i][0], cim[i][0]);
-                    Cw[(i * 8 + g) * LDP + 2 * t + 1] = cmake(cre[i][1], cim[i][1]);
-                }
-            }
-        }
-        __syncthreads();
-    }
+    __syncthreads();
 
     // ---- outputs, in exchanged (position) order
     for (int e = tid; e < n * B; e += NT) {
         int pos = e / B, c = e % B;
-        cplx v = panel[rowAt[pos] * LDP + c];
-        if (c < bw) Y[(long long)pos * n + k0 + c] = v;
-        if (pos == k0 + c) v.x -= 1.0;
-        Mult[(long long)pos * B + c] = v;
+        cplx v2 = panel[rowAt[pos] * LDP + c];
+        if (c < bw) Y[(long long)pos * n + k0 + c] = v2;
+        if (pos == k0 + c) v2.x -= 1.0;
+        Mult[(long long)pos * B + c] = v2;
     }
     // orig[pos] <- orig[rowAt[pos]]; rowAt for the update kernel
     int o = 0;
