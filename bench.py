@@ -34,9 +34,19 @@ sys.path.insert(0, ROOT)
 
 from paper_1107_5300_b200 import inputs  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the headline launch configuration,
-# from the ncu --set full capture summarised in profiles/ (bytes; None = not captured for this formulation)
-TRAFFIC_NCU = {"half": 68.63e9, "dense": None}      # profiles/ncu_r01_half_sweep.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the headline launch configuration: it
+# cannot be measured inside a timed run, so it is READ from the committed ncu --set full summary (its `dram_bytes_per_launch:` line)
+TRAFFIC_PROFILE = os.path.join("profiles", "ncu_r02_half_sweep.md")
+
+
+def traffic_from_profile():
+    try:
+        for line in open(os.path.join(ROOT, TRAFFIC_PROFILE)):
+            if line.startswith("dram_bytes_per_launch:"):
+                return float(line.split(":")[1])
+    except OSError:
+        pass
+    return None
 
 METRIC = "rgf_slice_steps_per_s"
 UNIT = "slice-steps/s"
@@ -335,7 +345,8 @@ def main():
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": peak,
-                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": TRAFFIC_NCU.get(a.form) if (w.M, w.L, n_E) == (244, 8000, 512) else None,
+                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": traffic_from_profile() if (a.form, w.M, w.L, n_E) == ("half", 244, 8000, 512) else None,
+                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, " + TRAFFIC_PROFILE,
                          "peak_source": "measured live: rgf_fp64_peak_tflops (DMMA issue rate, this GPU)",
                          "launches_timed": n_upd, "share_of_step": ms_upd / ms if ms else None},
         }
