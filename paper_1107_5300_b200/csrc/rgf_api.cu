@@ -41,12 +41,9 @@ struct Buf {
 
 }  // namespace
 
-// Per-stream workspace: one cohort of matrices runs all its slices on one stream; cohorts on
-// different streams overlap (the latency-bound panel kernel of one with the DMMA update of another).
+// Workspace of the sweep (one per plan, on the plan's stream): cohorts of matrices run one after the other.
 struct Ws {
     cudaStream_t stream = nullptr;
-    bool own_stream = false;
-    cudaEvent_t done = nullptr;
     Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
     Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm, Cp0, Cp1;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
@@ -65,7 +62,7 @@ struct rgf_plan {
     Buf pivmin, gsq, T_keep, redo_idx;                 // near-neutrality guard: smallest pivot per matrix, first-pass T, redone energies
     std::vector<double> guard_G, guard_Gmax;      // rms over the B half-steps / max of |t| / smallest pivot, per batch item of the last call
     double guard_tol = 1e-10;
-    std::vector<Ws> ws;                           // ws[0] runs on the plan's stream
+    std::vector<Ws> ws;                           // one workspace, on the plan's stream
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
@@ -75,7 +72,6 @@ struct rgf_plan {
     Buf lead_status;                              // [n_E] bad pivot inside the lead decimation of an energy
     int lead_method = RGF_LEAD_MODE_SPACE;
     int cohort_override = 0;
-    int nstreams = 1;
     int profiling = 0;
     int formulation = RGF_FORM_HALF;
     int precision = RGF_C128;                     // of the call in progress
@@ -157,16 +153,13 @@ int launch_zgemm(rgf_plan *p, cudaStream_t stream, const ZgemmArgs &a, int batch
     return RGF_OK;
 }
 
-int ensure_ws_streams(rgf_plan *p)
+// the plan's one workspace runs on the plan's stream
+int ensure_ws(rgf_plan *p)
 {
-    if ((int)p->ws.size() == p->nstreams) return RGF_OK;
-    for (size_t i = p->ws.size(); i < (size_t)p->nstreams; i++) {
-        Ws w;
-        if (i == 0) { w.stream = p->stream; }
-        else { CUDA_TRY(p, cudaStreamCreateWithFlags(&w.stream, cudaStreamNonBlocking)); w.own_stream = true; }
-        CUDA_TRY(p, cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
-        p->ws.push_back(w);
-    }
+    if (!p->ws.empty()) return RGF_OK;
+    Ws w;
+    w.stream = p->stream;
+    p->ws.push_back(w);
     return RGF_OK;
 }
 
@@ -501,7 +494,7 @@ int choose_cohort(const rgf_plan *p, int batch)
 {
     if (use_fused(p) && p->precision == RGF_C128) return batch;      // fused kernel: rgf_set_cohort bounds the units per launch instead
     if (p->cohort_override > 0) return std::min(p->cohort_override, batch);
-    return (batch + p->nstreams - 1) / p->nstreams;      // one cohort per stream
+    return batch;                                         // one cohort
 }
 
 int ensure_sweep_ws(rgf_plan *p, Ws &w, int cohort)
@@ -767,7 +760,7 @@ int begin_call(rgf_plan *p)
     if (!p) return RGF_EINVAL;
     p->err[0] = 0;
     CUDA_TRY(p, cudaSetDevice(p->device));
-    int rc = ensure_ws_streams(p);
+    int rc = ensure_ws(p);
     if (rc) return rc;
     return set_kernel_attrs(p);
 }
@@ -1030,8 +1023,6 @@ int rgf_destroy(rgf_plan *p)
         Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm, &w.Cp0, &w.Cp1};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
-        if (w.done) cudaEventDestroy(w.done);
-        if (w.own_stream && w.stream) cudaStreamDestroy(w.stream);
     }
     for (int i = 0; i < 5; i++) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);

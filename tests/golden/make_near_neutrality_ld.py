@@ -14,6 +14,9 @@ Green's function is the stable root of a quadratic (no iteration, no resonance).
 tests/test_oracle_pins.py pins it to the oracle away from E = 0 and to the closed-form T of the clean ribbon.
 
     python tests/golden/make_near_neutrality_ld.py [case ...]      (minutes per disordered case)
+    python tests/golden/make_near_neutrality_ld.py --config3 IDX [IDX ...]
+        the same evaluation for energies of the disordered configs[3] ribbon (M = 244, L = 2000; 35 minutes per energy),
+        appended to tests/golden/config3_ld.txt: the referee for the half-slice formulation's guard at resonant energies
 """
 import os
 import sys
@@ -118,7 +121,23 @@ def transmission_ld(onsite, vac, t, E, eta):
     return float(np.trace(GL @ (P.conj().T @ GR @ P)).real)
 
 
+def main_config3(indices):
+    w = inputs.config3(disordered=True)
+    out = os.path.join(HERE, "config3_ld.txt")
+    if not os.path.exists(out):
+        with open(out, "w") as f:
+            f.write("# T(E) of the disordered configs[3] ribbon (M=244 L=2000 W=0.1 seed 5301) in 80-bit arithmetic, written by\n"
+                    "# tests/golden/make_near_neutrality_ld.py --config3 (numpy %s); t=-2.7 eV eta=1e-9 eV\n# columns: energy_index E[eV] T\n" % np.__version__)
+    for k in indices:
+        T = transmission_ld(w.onsite[0], None, w.t, w.energies[k], w.eta)
+        with open(out, "a") as f:
+            f.write("%d %.17g %.17g\n" % (k, w.energies[k], T))
+        print(k, w.energies[k], T, flush=True)
+
+
 def main():
+    if len(sys.argv) > 1 and sys.argv[1] == "--config3":
+        return main_config3([int(x) for x in sys.argv[2:]])
     cases = sys.argv[1:] or list(inputs.NEAR_NEUTRALITY_CASES)
     out = os.path.join(HERE, "near_neutrality_ld.txt")
     old = {}

@@ -68,6 +68,24 @@ def test_config3_disordered_c128(plan):
     check(w, T, 3)
 
 
+def test_config3_resonant_energies_against_80bit(plan):
+    """configs[3], disordered, at energies inside the disorder band where the half-slice formulation alone is off by 2e-9 ... 4e-9
+    (its singly bonded atoms are resonant at many slices) and the guard must hand the energy to the dense formulation: the
+    default formulation, whole 1024-energy batch as bench-style runs launch it, against tests/golden/config3_ld.txt (80-bit
+    arithmetic, written by tests/golden/make_near_neutrality_ld.py --config3: neither oracle nor CUDA)."""
+    path = os.path.join(GOLDEN, "config3_ld.txt")
+    rows = np.loadtxt(path, ndmin=2)
+    idx, E, T_ld = rows[:, 0].astype(int), rows[:, 1], rows[:, 2]
+    assert len(idx) >= 2
+    w = inputs.config3(disordered=True)
+    assert np.array_equal(w.energies[idx], E)
+    plan.set_device(w.onsite, w.t)
+    T = plan.transmission(w.energies, w.eta)[0]
+    assert plan.stats()["guard_redone"] >= len(idx)
+    err = np.abs(T[idx] - T_ld) / np.maximum(1.0, T_ld)
+    assert np.all(err <= 1e-9), (err, T[idx], T_ld)
+
+
 def test_config3_clean_c128_closed_form(plan):
     """configs[3] variant (a): clean M=244, L=2000 against the closed form (skip points within 1e-4 eV of a subband edge, Q8)."""
     from test_oracle_pins import closed_form_T
