@@ -41,9 +41,11 @@ struct Buf {
 
 }  // namespace
 
-// Workspace of the sweep (one per plan, on the plan's stream): cohorts of matrices run one after the other.
+// Workspace of the sweep.  ws[0] runs on the plan's stream: cohorts of matrices one after the other.  ws[1] has a stream
+// of its own and is used by the guard pass only, whose two sweeps (from either lead) run side by side (run_dense_two_sided).
 struct Ws {
     cudaStream_t stream = nullptr;
+    bool own_stream = false;
     Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
     Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm, Cp0, Cp1;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
@@ -62,7 +64,9 @@ struct rgf_plan {
     Buf pivmin, gsq, T_keep, redo_idx;                 // near-neutrality guard: smallest pivot per matrix, first-pass T, redone energies
     std::vector<double> guard_G, guard_Gmax;      // rms over the B half-steps / max of |t| / smallest pivot, per batch item of the last call
     double guard_tol = 1e-10;
-    std::vector<Ws> ws;                           // one workspace, on the plan's stream
+    std::vector<Ws> ws;                           // two workspaces (see Ws)
+    cudaEvent_t ev_sync[2] = {nullptr, nullptr};  // fork / join of the guard pass's second stream
+    Buf jn[1];                                    // junction of the two sweeps: the block of gR the central slice couples to
     Buf gL, gR;                                   // lead surface Green's functions [n_E][M][M]
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
@@ -157,9 +161,13 @@ int launch_zgemm(rgf_plan *p, cudaStream_t stream, const ZgemmArgs &a, int batch
 int ensure_ws(rgf_plan *p)
 {
     if (!p->ws.empty()) return RGF_OK;
-    Ws w;
+    Ws w, w2;
     w.stream = p->stream;
+    CUDA_TRY(p, cudaStreamCreateWithFlags(&w2.stream, cudaStreamNonBlocking));
+    w2.own_stream = true;
+    for (int k = 0; k < 2; k++) CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_sync[k], cudaEventDisableTiming));
     p->ws.push_back(w);
+    p->ws.push_back(w2);
     return RGF_OK;
 }
 
@@ -551,6 +559,109 @@ int run_sweep_cohort(rgf_plan *p, Ws &w, int n_E, double eta, int bz0, int nb, i
     return RGF_OK;
 }
 
+int run_trace_cohort(rgf_plan *p, Ws &w, int n_E, int bz0, int nb, cplx *scratch, cplx *Pcur);
+
+// The dense formulation swept from BOTH leads at once, for the guard pass: a handful of matrices, where the time is the
+// sequential latency of the slices (0.5 ms each), not throughput.  Left chain (plan's stream): slices 0 .. m with
+// P_m = G^L_{m,0}; right chain (second stream, side by side on the idle SMs): slices L-1 .. c+1, c = m + 1, with
+// Q = G^R_{c+1,L-1}; both are lead-connected, hence as stable as the one-sided sweep.  They meet at the central slice c, which
+// is added like any slice of the one-sided sweep, the right part standing in for a lead:
+//     G_cc = (z - H_c - V_m gL_m V_m - V_c gR_{c+1} V_c)^-1,   G_{c,0} = G_cc V_m P_m,   G_{L-1,0} = Q^T V_c G_{c,0}   (G = G^T)
+// (Dyson's equation, Eq. 3), then the trace as usual.  Every block that is multiplied connects the two
+// sublattices; the closed form that joins the two surfaces directly, (1 - gL V gR V)^-1, contains the same-sublattice blocks
+// of two terminated halves, which diverge like 1/E towards charge neutrality, and lost 5e-9 at |E| = 4e-3 eV (measured).
+// Half the sequential steps.  Covers the cohort [bz0, bz0 + nb); writes p->T.
+int run_dense_two_sided(rgf_plan *p, int n_E, double eta, int bz0, int nb)
+{
+    const int M = p->M, L = p->L, nh = p->nh, m = L / 2 - 1;
+    Ws &wl = p->ws[0], &wr = p->ws[1];
+    int rc;
+    if ((rc = ensure_sweep_ws(p, wl, nb)) || (rc = ensure_sweep_ws(p, wr, nb))) return rc;
+    const size_t hb = sizeof(cplx) * (size_t)nh * nh * nb;
+    for (Buf &b : p->jn) if ((rc = ensure(p, b, hb))) return rc;
+    int *status = ptr<int>(p->status) + bz0;
+    const double *E = ptr<double>(p->E);
+    const long long hs = (long long)nh * nh, MM = (long long)M * M;
+    cplx *GL = ptr<cplx>(wl.G0), *GLalt = ptr<cplx>(wl.G1), *Pcur = ptr<cplx>(wl.Pa), *Pnext = ptr<cplx>(wl.Pb);
+    cplx *GR = ptr<cplx>(wr.G0), *GRalt = ptr<cplx>(wr.G1), *Qcur = ptr<cplx>(wr.Pa), *Qnext = ptr<cplx>(wr.Pb);
+    dim3 ag((unsigned)std::min<long long>((MM + 255) / 256, 2048), nb), pg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
+    const int nR = half_count(M, (L - 1) & 1);
+    auto masked_gemm = [&](cudaStream_t st, const cplx *A, long long a_batch, long long a_rs, long long a_cs, int mask_row, const cplx *B,
+                           cplx *C, int Mr, int K, int Nc, double alpha) -> int {
+        ZgemmArgs a;
+        memset(&a, 0, sizeof(a));
+        a.A = A; a.a_batch = a_batch; a.a_rs = a_rs; a.a_cs = a_cs; a.kmask_div = 1;
+        if (mask_row >= 0) {
+            a.kmask = ptr<uint8_t>(p->bondc) + (long long)mask_row * nh;
+            a.kmask_batch = (long long)(L + 1) * nh; a.kmask_div = n_E; a.kmask_b0 = bz0;
+        }
+        a.B = B; a.b_batch = hs; a.ldb = nh;
+        a.C = C; a.c_batch = hs; a.ldc = nh;
+        a.Mr = Mr; a.K = K; a.Nc = Nc; a.alpha = cmake(alpha, 0.0);
+        return launch_zgemm(p, st, a, nb);
+    };
+    auto left_step = [&](int i) -> int {
+        assemble_kernel<<<ag, 256, 0, wl.stream>>>(GL, M, L, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                  ptr<uint8_t>(p->hop), ptr<cplx>(p->gL), lead_gR(p));
+        p->stats.launches++;
+        cplx *res = nullptr;
+        int r2 = run_inverse(p, wl, GL, GLalt, M, nb, status, &res);
+        if (r2) return r2;
+        if (res != GL) std::swap(GL, GLalt);
+        if (i == 0) {
+            propagator_start_kernel<<<pg, 256, 0, wl.stream>>>(GL, Pcur, M, nh);
+            p->stats.launches++;
+            return RGF_OK;
+        }
+        const int pi = i & 1, pp = (i - 1) & 1;      // P_i[S_i, :] = t g_i[S_i, S_{i-1}] m'_{i-1} P_{i-1}
+        r2 = masked_gemm(wl.stream, GL + (long long)pi * M + pp, MM, 2LL * M, 2, i, Pcur, Pnext, half_count(M, pi), half_count(M, pp), M / 2, p->t);
+        std::swap(Pcur, Pnext);
+        return r2;
+    };
+    auto right_step = [&](int i) -> int {
+        assemble_right_kernel<<<ag, 256, 0, wr.stream>>>(GR, M, L, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                        ptr<uint8_t>(p->hop), lead_gR(p));
+        p->stats.launches++;
+        cplx *res = nullptr;
+        int r2 = run_inverse(p, wr, GR, GRalt, M, nb, status, &res);
+        if (r2) return r2;
+        if (res != GR) std::swap(GR, GRalt);
+        const int pr = (i - 1) & 1, pc = i & 1;      // rows: atoms bonded to slice i - 1; Q_i = t gR_i[., S_i] m'_i Q_{i+1}
+        if (i == L - 1) {
+            block_extract_kernel<<<pg, 256, 0, wr.stream>>>(GR, Qcur, M, nh, pr, pc);
+            p->stats.launches++;
+            return RGF_OK;
+        }
+        r2 = masked_gemm(wr.stream, GR + (long long)pr * M + pc, MM, 2LL * M, 2, i + 1, Qcur, Qnext, half_count(M, pr), half_count(M, pc), nR, p->t);
+        std::swap(Qcur, Qnext);
+        return r2;
+    };
+    CUDA_TRY(p, cudaEventRecord(p->ev_sync[0], p->stream));
+    CUDA_TRY(p, cudaStreamWaitEvent(wr.stream, p->ev_sync[0], 0));
+    const int nl = m + 1, nr = L - 2 - m;          // the central slice c = m + 1 belongs to neither chain
+    for (int s = 0; s < std::max(nl, nr); s++) {
+        if (s < nl && (rc = left_step(s))) return rc;
+        if (s < nr && (rc = right_step(L - 1 - s))) return rc;
+    }
+    CUDA_TRY(p, cudaGetLastError());
+    CUDA_TRY(p, cudaEventRecord(p->ev_sync[1], wr.stream));
+    CUDA_TRY(p, cudaStreamWaitEvent(p->stream, p->ev_sync[1], 0));
+    // ---- central slice c and the junction, on the plan's stream
+    const int c = m + 1, pc = c & 1, pm = m & 1;
+    cplx *J0 = ptr<cplx>(p->jn[0]);
+    block_extract_kernel<<<pg, 256, 0, wl.stream>>>(GR, J0, M, nh, pc, pc);                // the block of gR_{c+1} that V_c keeps
+    ldos_assemble_kernel<<<ag, 256, 0, wl.stream>>>(GLalt, M, L, nh, c, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                   ptr<uint8_t>(p->hop), 1, GL, ptr<cplx>(p->gL), 1, J0, lead_gR(p));
+    p->stats.launches += 2;
+    cplx *Gcc = nullptr;
+    if ((rc = run_inverse(p, wl, GLalt, GL, M, nb, status, &Gcc))) return rc;
+    cplx *Gfree = (Gcc == GLalt) ? GL : GLalt;
+    if ((rc = masked_gemm(wl.stream, Gcc + (long long)pc * M + pm, MM, 2LL * M, 2, c, Pcur, Pnext, half_count(M, pc), half_count(M, pm), M / 2, p->t))) return rc;   // G_{c,0}
+    if ((rc = masked_gemm(wl.stream, Qcur, hs, 1, nh, c + 1, Pnext, Pcur, nR, half_count(M, pc), M / 2, p->t))) return rc;        // G_{L-1,0} = t Q^T m'_c G_{c,0}
+    CUDA_TRY(p, cudaGetLastError());
+    return run_trace_cohort(p, wl, n_E, bz0, nb, Gfree, Pcur);
+}
+
 // ---- half-slice formulation (half_kernels.cuh): 2 half-steps per slice, each an (M/2) inverse and an (M/2)^3 GEMM ----
 int ensure_sweep_ws_half(rgf_plan *p, Ws &w, int cohort)
 {
@@ -885,6 +996,9 @@ static int transmission_pass(rgf_plan *p, int n_E, double eta, int formulation, 
         if (half) {
             rc = run_sweep_cohort_half(p, w, n_E, eta, bz0, nb, p->L, &G, &Pcur);
             Galt = ptr<cplx>(w.Tr);
+        } else if (!first_pass && p->L >= 4) {
+            rc = run_dense_two_sided(p, n_E, eta, bz0, nb);          // includes the trace
+            continue;
         } else {
             rc = run_sweep_cohort(p, w, n_E, eta, bz0, nb, p->L, &G, &Galt, &Pcur);
         }
@@ -1023,8 +1137,11 @@ int rgf_destroy(rgf_plan *p)
         Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm, &w.Cp0, &w.Cp1};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+        if (w.own_stream && w.stream) cudaStreamDestroy(w.stream);
     }
     for (int i = 0; i < 5; i++) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    for (int i = 0; i < 2; i++) if (p->ev_sync[i]) cudaEventDestroy(p->ev_sync[i]);
+    for (Buf &b : p->jn) release(b);
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
     delete p;
     return RGF_OK;

@@ -47,6 +47,45 @@ __global__ void assemble_kernel(cplx *Gall, int M, int L, int i, int n_E, int bz
     }
 }
 
+// ---- the sweep from the right end (rgf_api.cu: run_dense_two_sided) -------------------------------------------------
+// gR_i = (z - H_i - t^2 m'_i (.) gR_{i+1} (.) m'_i)^-1, gR_L = surface Green's function of the right lead (Sigma_R at i = L-1):
+// the mirror image of assemble_kernel, written in place over gR_{i+1}.  Used for slices i >= 1 only (no Sigma_L).
+__global__ void assemble_right_kernel(cplx *Gall, int M, int L, int i, int n_E, int bz0, const double *energies, double eta, double t,
+                                      const double *onsite, const uint8_t *bond, const uint8_t *hop, const cplx *gR)
+{
+    const int bl = blockIdx.y, bz = bz0 + bl, d = bz / n_E, e = bz % n_E;
+    const long long MM = (long long)M * M;
+    cplx *G = Gall + (long long)bl * MM;
+    const double *eps = onsite + ((long long)d * L + i) * M;
+    const uint8_t *mnext = bond + ((long long)d * (L + 1) + i + 1) * M;      // m'_i: bond between slices i and i + 1
+    const uint8_t *hp = hop + ((long long)d * L + i) * M;
+    const double t2 = t * t;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < MM; idx += (long long)gridDim.x * blockDim.x) {
+        const int j = (int)(idx / M), k = (int)(idx % M);
+        cplx a = cmake(0.0, 0.0);
+        if (j == k) a = cmake(energies[e] - eps[j], eta);
+        else if (k == j + 1) { if (hp[j]) a.x = -t; }
+        else if (j == k + 1) { if (hp[k]) a.x = -t; }
+        if (mnext[j] && mnext[k]) {
+            const cplx g = (i == L - 1) ? gR[(long long)e * MM + idx] : G[idx];
+            a.x -= t2 * g.x; a.y -= t2 * g.y;
+        }
+        G[idx] = a;
+    }
+}
+
+// compact block of a full M x M matrix: Out[r][c] = G[2r + pr][2c + pc] (ld = nh), r < count(pr), c < count(pc)
+__global__ void block_extract_kernel(const cplx *Gall, cplx *Out, int M, int nh, int pr, int pc)
+{
+    const int bl = blockIdx.y, nr = (M - pr + 1) / 2, ncol = (M - pc + 1) / 2;
+    const cplx *G = Gall + (long long)bl * M * M;
+    cplx *O = Out + (long long)bl * nh * nh;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nr * ncol; idx += gridDim.x * blockDim.x) {
+        const int r = idx / ncol, c = idx % ncol;
+        O[(long long)r * nh + c] = G[(long long)(2 * r + pr) * M + 2 * c + pc];
+    }
+}
+
 // P_0 = g_0 restricted to rows S_0 and columns S_{-1} (compact nh x nh storage, ld = nh).
 __global__ void propagator_start_kernel(const cplx *Gall, cplx *Pall, int M, int nh)
 {

@@ -471,3 +471,33 @@ def test_ldos_device_pointers_and_chunks(rgf, plan, oracle):
     rgf.rgf_ldos(plan.handle, E_dev, 6, 2e-3, out)
     ref = oracle.ldos_batch(on, None, -2.7, E, 2e-3)
     assert np.max(np.abs(out.cpu().numpy()[0] - ref)) <= 1e-9 * max(1.0, np.max(ref))
+
+
+@pytest.mark.parametrize("M,L", [(23, 41), (20, 5), (23, 4)])
+def test_guard_pass_two_sided_sweep_odd_sizes(rgf, plan, oracle, M, L):
+    """The guard's second pass sweeps the dense formulation from both leads and joins the two halves by Dyson's equation
+    (run_dense_two_sided): odd M (the two sublattice blocks differ in size), odd L (g_R is a lead of its own, the halves
+    differ in length), the shortest L it is used for, vacancies next to the junction.  Metallic clean ribbons (M + 1
+    divisible by 3) at small |E| force every energy into that pass; closed form and oracle referee."""
+    from test_oracle_pins import closed_form_T
+    on = np.zeros((L, M))
+    E = np.array([1e-3, -1e-3, 2e-4, -2e-4])
+    plan.set_device(on, -2.7)
+    T = plan.transmission(E, 1e-9)[0]
+    assert plan.stats()["guard_redone"] == 4
+    for e, tk in zip(E, T):
+        assert abs(tk - closed_form_T(M, L, e)[0]) < 1e-9, (e, tk)
+    # with disorder and a vacancy on either side of the junction slice m = L // 2 - 1
+    on = inputs.anderson(M, L, 0.05, 5 + M)
+    vac = np.zeros((L, M), dtype=np.uint8)
+    m = L // 2 - 1
+    vac[m, 2] = vac[m + 1, 5] = 1
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    plan.set_device(on, -2.7, vac)
+    E2 = np.array([4e-3, -4e-3, 2e-3])
+    rgf.rgf_set_guard(plan.handle, 1e-14)          # force the pass for every energy
+    T2 = plan.transmission(E2, 1e-9)[0]
+    assert plan.stats()["guard_redone"] == 3
+    rgf.rgf_set_guard(plan.handle, 1e-10)
+    T_or = oracle.transmission_batch(on, vac, -2.7, E2, 1e-9)
+    assert np.all(np.abs(T2 - T_or) <= tol(T_or)), np.abs(T2 - T_or)
