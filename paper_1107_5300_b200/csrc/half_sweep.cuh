@@ -413,19 +413,21 @@ __device__ __forceinline__ void hs_acc_store(const HSAcc<RG> &h, cplx *Cl, int l
         if (rr < n && cok) st256(Cl + (long long)rr * ld, h.re[i][0], h.im[i][0], h.re[i][1], h.im[i][1]);
     }
 }
-template <int RG, bool FULL>
+// FULL = number of k-steps of 4 in straight-line code (8: a full 32-column panel; 7: a panel of 25 .. 28 columns, the last one of
+// n = 122 is 26 wide), 0 = generic loop over kq steps
+template <int RG, int FULL>
 __device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, int r0, const cplx (&bb)[8], int kq)
 {
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const cplx *cA = panel + (r0 + g) * HS_LDP + t;
-    if (FULL) {
-        // straight-line code for a full 32-column panel: the A fragments of step q + 1 are loaded before the DMMAs of step q
+    if (FULL > 0) {
+        // straight-line code: the A fragments of step q + 1 are loaded before the DMMAs of step q
         cplx a[2][RG];
 #pragma unroll
         for (int i = 0; i < RG; i++) a[0][i] = cA[i * 8 * HS_LDP];
 #pragma unroll
-        for (int q = 0; q < 8; q++) {
-            if (q + 1 < 8) {
+        for (int q = 0; q < FULL; q++) {
+            if (q + 1 < FULL) {
 #pragma unroll
                 for (int i = 0; i < RG; i++) a[(q + 1) & 1][i] = cA[i * 8 * HS_LDP + (q + 1) * 4];
             }
@@ -447,7 +449,7 @@ __device__ __forceinline__ void hs_acc_compute(HSAcc<RG> &h, const cplx *panel, 
 }
 
 // Mult columns / R rows beyond the panel width are zero, so a narrow last panel only skips DMMAs (FULL = false).
-template <int RG, bool FULL, int TF>
+template <int RG, int FULL, int TF>
 __device__ __forceinline__ void hs_strip_update(const cplx *panel, const int *prow, cplx *Cg, int ld, int n, int col0, int ncols, int bw,
                                                 const HSXf &xf)
 {
@@ -557,14 +559,16 @@ __device__ __forceinline__ void hs_gauss_jordan(HSmem &sm, cplx *X, cplx *W, int
             cplx *Cg; int col0, ncols;
             const bool isx = strip_of(s, Cg, col0, ncols);
             const int tfs = tf ? (isx ? xtf : wtf) : 0;
-            // FULL = straight-line code over all eight k-steps: Mult columns / pivot rows beyond the panel width are zero,
-            // so a slightly narrow panel (n = 122: the last one is 26 wide) only adds DMMAs on zeros
-            const bool full = bw > HS_B - 12;
+            // straight-line code over 8 k-steps (bw > 28) or 7 (24 < bw <= 28: the last panel of n = 122 is 26 wide); Mult columns /
+            // pivot rows beyond the panel width are zero, so a k-step that is only partly filled just adds DMMAs on zeros
+            const int full = bw > 28 ? 8 : (bw > 24 ? 7 : 0);
 #define HS_STRIP(F, T) hs_strip_update<HS_RG, F, T>(sm.panel, sm.prow, Cg, ld, n, col0, ncols, bw, xf)
-            if (full) {
-                if (tfs == 0) HS_STRIP(true, 0); else if (tfs == 1) HS_STRIP(true, 1); else if (tfs == 2) HS_STRIP(true, 2); else HS_STRIP(true, 3);
+            if (full == 8) {
+                if (tfs == 0) HS_STRIP(8, 0); else if (tfs == 1) HS_STRIP(8, 1); else if (tfs == 2) HS_STRIP(8, 2); else HS_STRIP(8, 3);
+            } else if (full == 7 && tfs == 0) {
+                HS_STRIP(7, 0);
             } else {
-                if (tfs == 0) HS_STRIP(false, 0); else if (tfs == 1) HS_STRIP(false, 1); else if (tfs == 2) HS_STRIP(false, 2); else HS_STRIP(false, 3);
+                if (tfs == 0) HS_STRIP(0, 0); else if (tfs == 1) HS_STRIP(0, 1); else if (tfs == 2) HS_STRIP(0, 2); else HS_STRIP(0, 3);
             }
 #undef HS_STRIP
         }
