@@ -583,6 +583,177 @@ static int ldos_sweep(int M, int L, const double *onsite, const uint8_t *vac, do
     return rc;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * O10. The paper's own form of the recursion, in double or in IEEE single precision
+ * (SURVEY.md 8(c) "Precision finding"; Eq. 4, Eq. 5).
+ *   G0_j  = (z - H_j [- Sigma_L at j = 0] [- Sigma_R at j = L-1])^-1      Green's function of the isolated slice
+ *   G_jj  = (1 - G0_j V G_{j-1,j-1} V)^-1 G0_j                             Eq. 4 (Sigma^l, Sigma^r of the paper = the hopping V)
+ *   G_j0  = G_jj V G_{j-1,0}                                               Eq. 5 in the column form (reading Q4)
+ * Algebraically the same as the direct form of sweep(); numerically not: G0_j is ill-conditioned whenever E is near a
+ * level of the isolated slice.  use_float = 1 runs every matrix operation of the sweep and the trace in single precision
+ * (own float LU and matmul below); the lead self-energies are computed in double and rounded (reading Q17: the paper
+ * computed them on the CPU).  This reproduces the paper's single-precision finding on the CPU; it is not compared with
+ * the CUDA path, whose complex64 sweep uses the direct form.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { float re, im; } cplxf;
+static inline cplxf f_make(float re, float im) { cplxf r; r.re = re; r.im = im; return r; }
+static inline cplxf f_add(cplxf a, cplxf b) { return f_make(a.re + b.re, a.im + b.im); }
+static inline cplxf f_sub(cplxf a, cplxf b) { return f_make(a.re - b.re, a.im - b.im); }
+static inline cplxf f_mul(cplxf a, cplxf b) { return f_make(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
+static inline cplxf f_div(cplxf a, cplxf b)
+{
+    if (fabsf(b.re) >= fabsf(b.im)) {
+        float r = b.im / b.re, d = b.re + b.im * r;
+        return f_make((a.re + a.im * r) / d, (a.im - a.re * r) / d);
+    } else {
+        float r = b.re / b.im, d = b.re * r + b.im;
+        return f_make((a.re * r + a.im) / d, (a.im * r - a.re) / d);
+    }
+}
+
+static void mat_mul_f(int n, const cplxf *A, const cplxf *B, cplxf *C)
+{
+    for (int i = 0; i < n; i++) {
+        cplxf *Ci = C + (size_t)i * n;
+        for (int j = 0; j < n; j++) Ci[j] = f_make(0.f, 0.f);
+        for (int k = 0; k < n; k++) {
+            cplxf a = A[(size_t)i * n + k];
+            const cplxf *Bk = B + (size_t)k * n;
+            for (int j = 0; j < n; j++) Ci[j] = f_add(Ci[j], f_mul(a, Bk[j]));
+        }
+    }
+}
+
+/* the LU of mat_inverse, in single precision (the paper's CGESV) */
+static int mat_inverse_f(int n, const cplxf *A, cplxf *Ainv)
+{
+    cplxf *LU = (cplxf *)malloc(sizeof(cplxf) * (size_t)n * n);
+    int *perm = (int *)malloc(sizeof(int) * (size_t)n);
+    cplxf *y = (cplxf *)malloc(sizeof(cplxf) * (size_t)n);
+    if (!LU || !perm || !y) { free(LU); free(perm); free(y); return ORC_ENOMEM; }
+    memcpy(LU, A, sizeof(cplxf) * (size_t)n * n);
+    for (int i = 0; i < n; i++) perm[i] = i;
+    int rc = ORC_OK;
+    for (int k = 0; k < n; k++) {
+        int p = k;
+        float best = LU[(size_t)k * n + k].re * LU[(size_t)k * n + k].re + LU[(size_t)k * n + k].im * LU[(size_t)k * n + k].im;
+        for (int i = k + 1; i < n; i++) {
+            cplxf x = LU[(size_t)i * n + k];
+            float v = x.re * x.re + x.im * x.im;
+            if (v > best) { best = v; p = i; }
+        }
+        if (!(best > 0.f) || !isfinite(best)) { rc = ORC_ESINGULAR; break; }
+        if (p != k) {
+            for (int j = 0; j < n; j++) { cplxf tmp = LU[(size_t)k * n + j]; LU[(size_t)k * n + j] = LU[(size_t)p * n + j]; LU[(size_t)p * n + j] = tmp; }
+            int tp = perm[k]; perm[k] = perm[p]; perm[p] = tp;
+        }
+        cplxf piv = LU[(size_t)k * n + k];
+        for (int i = k + 1; i < n; i++) {
+            cplxf f = f_div(LU[(size_t)i * n + k], piv);
+            LU[(size_t)i * n + k] = f;
+            cplxf *Li = LU + (size_t)i * n;
+            const cplxf *Lk = LU + (size_t)k * n;
+            for (int j = k + 1; j < n; j++) Li[j] = f_sub(Li[j], f_mul(f, Lk[j]));
+        }
+    }
+    if (rc == ORC_OK) {
+        for (int c = 0; c < n; c++) {
+            for (int i = 0; i < n; i++) {
+                cplxf sacc = (perm[i] == c) ? f_make(1.f, 0.f) : f_make(0.f, 0.f);
+                const cplxf *Li = LU + (size_t)i * n;
+                for (int j = 0; j < i; j++) sacc = f_sub(sacc, f_mul(Li[j], y[j]));
+                y[i] = sacc;
+            }
+            for (int i = n - 1; i >= 0; i--) {
+                cplxf sacc = y[i];
+                const cplxf *Ui = LU + (size_t)i * n;
+                for (int j = i + 1; j < n; j++) sacc = f_sub(sacc, f_mul(Ui[j], y[j]));
+                y[i] = f_div(sacc, Ui[i]);
+            }
+            for (int i = 0; i < n; i++) Ainv[(size_t)i * n + c] = y[i];
+        }
+    }
+    free(LU); free(perm); free(y);
+    return rc;
+}
+
+/* One body for the two precisions: CT = complex type, RT = real type, and its helpers. */
+#define ORC_EQ4_SWEEP(NAME, CT, RT, MK, ADD, SUB, MATMUL, MATINV)                                                          \
+static int NAME(int M, int L, const double *onsite, const uint8_t *vac, double t, double E, double eta, int lead_method,  \
+                double *T_out)                                                                                             \
+{                                                                                                                          \
+    size_t MM = (size_t)M * M;                                                                                             \
+    cplx z = c_make(E, eta);                                                                                               \
+    cplx *SigL = (cplx *)malloc(sizeof(cplx) * MM * 3), *SigR = SigL ? SigL + MM : NULL, *H = SigL ? SigL + 2 * MM : NULL;   \
+    CT *buf = (CT *)malloc(sizeof(CT) * MM * 8);                                                                           \
+    double *mp = (double *)malloc(sizeof(double) * (size_t)M);                                                             \
+    if (!SigL || !buf || !mp) { free(SigL); free(buf); free(mp); return ORC_ENOMEM; }                                      \
+    CT *A = buf, *G0 = buf + MM, *g = buf + 2 * MM, *gprev = buf + 3 * MM, *P = buf + 4 * MM, *Pprev = buf + 5 * MM,       \
+       *X = buf + 6 * MM, *Y = buf + 7 * MM;                                                                               \
+    int rc = lead_self_energy(M, L, vac, t, z, -1, lead_method, SigL, NULL);                                               \
+    if (rc == ORC_OK) rc = lead_self_energy(M, L, vac, t, z, +1, lead_method, SigR, NULL);                                 \
+    for (int i = 0; i < L && rc == ORC_OK; i++) {                                                                          \
+        slice_hamiltonian(M, L, onsite, vac, i, t, H);                                                                     \
+        for (size_t k = 0; k < MM; k++) {                       /* z - H_i - lead self-energy, formed in double, rounded */ \
+            cplx v = c_make(-H[k].re, -H[k].im);                                                                           \
+            if (k / M == k % M) v = c_add(v, z);                                                                           \
+            if (i == 0) v = c_sub(v, SigL[k]);                                                                             \
+            if (i == L - 1) v = c_sub(v, SigR[k]);                                                                         \
+            A[k] = MK((RT)v.re, (RT)v.im);                                                                                 \
+        }                                                                                                                  \
+        rc = MATINV(M, A, G0);                                  /* G0_j of the isolated slice */                           \
+        if (rc != ORC_OK) break;                                                                                           \
+        if (i == 0) {                                                                                                      \
+            memcpy(g, G0, sizeof(CT) * MM);                                                                                \
+            memcpy(P, g, sizeof(CT) * MM);                                                                                 \
+        } else {                                                                                                           \
+            bond_mask(M, L, vac, i - 1, mp);                                                                               \
+            for (int r = 0; r < M; r++)                         /* X = V G_{j-1,j-1} V */                                  \
+                for (int c = 0; c < M; c++) {                                                                              \
+                    RT sc = (RT)((t * mp[r]) * (t * mp[c]));                                                               \
+                    X[(size_t)r * M + c] = MK(gprev[(size_t)r * M + c].re * sc, gprev[(size_t)r * M + c].im * sc);         \
+                }                                                                                                          \
+            MATMUL(M, G0, X, Y);                                /* G0 V G V */                                             \
+            for (size_t k = 0; k < MM; k++) Y[k] = MK(-Y[k].re, -Y[k].im);                                                 \
+            for (int d = 0; d < M; d++) Y[(size_t)d * M + d] = ADD(Y[(size_t)d * M + d], MK((RT)1, (RT)0));                \
+            rc = MATINV(M, Y, X);                               /* (1 - G0 V G V)^-1 */                                    \
+            if (rc != ORC_OK) break;                                                                                       \
+            MATMUL(M, X, G0, g);                                /* Eq. 4 */                                                \
+            for (int r = 0; r < M; r++)                                                                                    \
+                for (int c = 0; c < M; c++) {                                                                              \
+                    RT sc = (RT)(t * mp[c]);                                                                               \
+                    X[(size_t)r * M + c] = MK(g[(size_t)r * M + c].re * sc, g[(size_t)r * M + c].im * sc);                 \
+                }                                                                                                          \
+            MATMUL(M, X, Pprev, P);                             /* Eq. 5 */                                                \
+        }                                                                                                                  \
+        memcpy(gprev, g, sizeof(CT) * MM);                                                                                 \
+        memcpy(Pprev, P, sizeof(CT) * MM);                                                                                 \
+    }                                                                                                                      \
+    if (rc == ORC_OK) {                                         /* Eq. 2 in the sweep's precision */                       \
+        CT *GamL = A, *GamR = G0;                                                                                          \
+        for (int r = 0; r < M; r++)                                                                                        \
+            for (int c = 0; c < M; c++) {                                                                                  \
+                cplx a = SigL[(size_t)r * M + c], b = SigL[(size_t)c * M + r];                                             \
+                GamL[(size_t)r * M + c] = MK((RT)(-(a.im + b.im)), (RT)(a.re - b.re));                                     \
+                a = SigR[(size_t)r * M + c]; b = SigR[(size_t)c * M + r];                                                  \
+                GamR[(size_t)r * M + c] = MK((RT)(-(a.im + b.im)), (RT)(a.re - b.re));                                     \
+            }                                                                                                              \
+        MATMUL(M, GamR, Pprev, X);                                                                                         \
+        for (int r = 0; r < M; r++)                                                                                        \
+            for (int c = 0; c < M; c++) Y[(size_t)r * M + c] = MK(Pprev[(size_t)c * M + r].re, -Pprev[(size_t)c * M + r].im); \
+        MATMUL(M, Y, X, P);                                                                                                \
+        MATMUL(M, GamL, P, X);                                                                                             \
+        double tr = 0.0;                                                                                                   \
+        for (int d = 0; d < M; d++) tr += (double)X[(size_t)d * M + d].re;                                                 \
+        *T_out = tr;                                                                                                       \
+    }                                                                                                                      \
+    free(SigL); free(buf); free(mp);                                                                                       \
+    return rc;                                                                                                             \
+}
+
+ORC_EQ4_SWEEP(sweep_eq4_d, cplx, double, c_make, c_add, c_sub, mat_mul, mat_inverse)
+ORC_EQ4_SWEEP(sweep_eq4_f, cplxf, float, f_make, f_add, f_sub, mat_mul_f, mat_inverse_f)
+
 /* ==========================================================================================
  * Exported C ABI of the oracle (loaded through ctypes by oracle/rgf_oracle.py).
  * Complex arrays: interleaved doubles, row-major.
@@ -689,6 +860,32 @@ int orc_ldos_batch(int M, int L, const double *onsite, const uint8_t *vac, doubl
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
     for (int k = 0; k < n_E; k++) {
         int rc = ldos_sweep(M, L, onsite, vac, t, energies[k], eta, lead_method, ldos_out + (size_t)k * L * M);
+        if (rc != ORC_OK) {
+#pragma omp critical
+            { if (first == ORC_OK) first = rc; }
+        }
+    }
+    return first;
+}
+
+/* T(E) by the paper's Eq. 4 form (O10), in double (use_float = 0) or IEEE single precision (1); OpenMP over energies. */
+int orc_transmission_eq4_batch(int M, int L, const double *onsite, const uint8_t *vac, double t, const double *energies, int n_E,
+                               double eta, int use_float, int lead_method, int nthreads, double *T_out, int *status)
+{
+    if (M < 2 || L < 1 || n_E < 1 || !(eta > 0.0) || !onsite || !energies || !T_out) return ORC_EINVAL;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+    int first = ORC_OK;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int k = 0; k < n_E; k++) {
+        double T = NAN;
+        int rc = use_float ? sweep_eq4_f(M, L, onsite, vac, t, energies[k], eta, lead_method, &T)
+                           : sweep_eq4_d(M, L, onsite, vac, t, energies[k], eta, lead_method, &T);
+        T_out[k] = (rc == ORC_OK) ? T : NAN;
+        if (status) status[k] = rc;
         if (rc != ORC_OK) {
 #pragma omp critical
             { if (first == ORC_OK) first = rc; }

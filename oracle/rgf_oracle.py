@@ -34,6 +34,7 @@ def lib():
         L.orc_transmission.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, dp, dp, ip]
         L.orc_sweep_state.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, dp, dp]
         L.orc_transmission_batch.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, dp, C.c_int, C.c_double, C.c_int, C.c_int, dp, ip]
+        L.orc_transmission_eq4_batch.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, dp, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, dp, ip]
         L.orc_ldos_batch.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, dp, C.c_int, C.c_double, C.c_int, C.c_int, dp]
         L.orc_transmission_brute.argtypes = [C.c_int, C.c_int, dp, u8p, C.c_double, C.c_double, C.c_double, C.c_int, dp, dp]
         _lib = L
@@ -159,3 +160,14 @@ def ldos_batch(onsite, vacancy, t, energies, eta, method=LEAD_CELL, nthreads=0):
     if rc:
         raise OracleError(rc, "ldos_batch")
     return out
+
+
+def transmission_eq4_batch(onsite, vacancy, t, energies, eta, use_float, method=LEAD_CELL, nthreads=0):
+    """T(E) by the paper's own Eq. 4 form (O10), double or single precision; a failed energy is NaN."""
+    onsite, vac, vp, M, L = _onsite(onsite, vacancy)
+    E = np.ascontiguousarray(energies, dtype=np.float64)
+    T = np.empty(E.shape[0], dtype=np.float64)
+    st = np.zeros(E.shape[0], dtype=np.int32)
+    lib().orc_transmission_eq4_batch(M, L, _dp(onsite), vp, t, _dp(E), E.shape[0], eta, 1 if use_float else 0, method, nthreads, _dp(T),
+                                     st.ctypes.data_as(C.POINTER(C.c_int)))
+    return T

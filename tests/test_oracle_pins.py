@@ -432,3 +432,32 @@ def test_ldos_closed_forms_and_invariants(oracle):
     grid = np.linspace(-0.2, 0.2, 4001)
     w = oracle.ldos_batch(on1, v1, T_HOP, grid, 5e-3)[:, 1, 1]
     assert abs(np.trapezoid(w, grid) - 2 / np.pi * np.arctan(0.2 / 5e-3)) < 1e-6
+
+
+# ----------------------------------------------------------------------------------------
+# O10: the paper's own Eq. 4 form, double and single precision (SURVEY.md 8(c) "Precision finding")
+# ----------------------------------------------------------------------------------------
+
+def test_eq4_form_equals_direct_form_in_double(oracle):
+    """(1 - G0 V G V)^-1 G0 = (z - H - V G V)^-1: the two forms of Eq. 4 agree to rounding away from the levels of the
+    isolated slices (disorder, vacancies on both end slices, odd M and L)."""
+    M, L = 9, 7
+    on = inputs.anderson(M, L, 0.3, 31)
+    vac = np.zeros((L, M), dtype=np.uint8)
+    vac[0, 1] = vac[3, 0] = vac[L - 1, 4] = 1
+    on[vac != 0] = inputs.VACANCY_ONSITE
+    E = np.array([-1.3, -0.37, 0.21, 0.9])
+    T_direct = oracle.transmission_batch(on, vac, T_HOP, E, ETA)
+    T_eq4 = oracle.transmission_eq4_batch(on, vac, T_HOP, E, ETA, use_float=False)
+    assert np.max(np.abs(T_eq4 - T_direct)) < 1e-10
+
+
+def test_eq4_form_in_single_precision_is_single_precision(oracle):
+    """The float sweep (own float LU and matmul) lands within single-precision distance of the double one on a short benign
+    ribbon -- a wrong index or sign in the float routines would be O(1) off -- and is not the double result."""
+    w = inputs.config0(M=20, L=12, n_E=6)
+    E = w.energies + 0.0131
+    T_d = oracle.transmission_eq4_batch(w.onsite[0], None, w.t, E, w.eta, use_float=False)
+    T_f = oracle.transmission_eq4_batch(w.onsite[0], None, w.t, E, w.eta, use_float=True)
+    d = np.abs(T_f - T_d)
+    assert np.all(np.isfinite(T_f)) and d.max() < 1e-3 and d.max() > 1e-9
