@@ -71,7 +71,7 @@ struct rgf_plan {
     Buf l_eps, l_eps_s, l_alpha, l_beta, l_T1, l_T2, l_T3, l_W, l_W2;   // decimation workspace
     Buf stage_in, stage_out;                      // staging for host<->device of sub-step entry points
     Buf lc_S3, lc_R;                              // run_lead_side_schur: S again and the residual of its inverse
-    Buf ld_A0, ld_A1, ld_B0, ld_B1, ld_stash, ld_out;   // rgf_ldos: two inverse ping-pong pairs, the stashed gR blocks, the LDOS of a chunk
+    Buf ld_A0, ld_A1, ld_B0, ld_B1, ld_stash, ld_stashL, ld_out;   // rgf_ldos: batched G_ii work buffers, flags, the stashed gR / gL blocks, the LDOS of a chunk
     Buf lm_Q;                                     // mode-space leads: the orthogonal basis Q [nc][nc]
     Buf lead_status;                              // [n_E] bad pivot inside the lead decimation of an energy
     int lead_method = RGF_LEAD_MODE_SPACE;
@@ -1130,7 +1130,7 @@ int rgf_destroy(rgf_plan *p)
     if (p->stream) cudaStreamSynchronize(p->stream);
     Buf *bufs[] = {&p->onsite, &p->bond, &p->hop, &p->bondc, &p->E, &p->T, &p->status, &p->lead_flags, &p->pivmin, &p->gsq, &p->T_keep, &p->redo_idx,
                    &p->gL, &p->gR, &p->l_eps, &p->l_eps_s, &p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3,
-                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status, &p->ld_A0, &p->ld_A1, &p->ld_B0, &p->ld_B1, &p->ld_stash, &p->ld_out};
+                   &p->l_W, &p->l_W2, &p->stage_in, &p->stage_out, &p->lc_S3, &p->lc_R, &p->lm_Q, &p->lead_status, &p->ld_A0, &p->ld_A1, &p->ld_B0, &p->ld_B1, &p->ld_stash, &p->ld_stashL, &p->ld_out};
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
@@ -1369,8 +1369,9 @@ int rgf_unshard(const double *T_shard, int n_dev, int n_E, int world, int rank, 
 }
 
 // F-4: local density of states of the connected device, LDOS[n_dev][n_E][L][M] (ldos_kernels.cuh states the recursion).
-// Three batched M x M inverses per slice and matrix (gR_i on the way back, gL_i and G_ii on the way forth); the gR blocks
-// of a chunk of matrices are stashed in HBM between the two passes, the chunk sized to at most half of the free memory.
+// Three batched M x M inverses per slice and matrix: the gR chain and the gL chain run side by side on two streams and stash
+// their (M/2)-blocks in HBM; the G_ii of all slices are then inverted in batches of (matrix, slice) pairs.  Matrices in
+// chunks sized to at most half of the free memory.
 int rgf_ldos(rgf_plan *p, const double *energies, int n_E, double eta, double *ldos_out)
 {
     int rc = begin_call(p);
@@ -1389,52 +1390,72 @@ int rgf_ldos(rgf_plan *p, const double *energies, int n_E, double eta, double *l
     int lead_open = 0;
     if ((rc = run_leads(p, n_E, eta, &lead_open))) return rc;
     if (lead_open) return fail(p, RGF_ENOCONV, "lead decimation did not converge for %d energies", lead_open);
-    // chunk of matrices whose stash fits
+    // chunk of matrices whose two stashes fit
     size_t free_b = 0, total_b = 0;
     CUDA_TRY(p, cudaMemGetInfo(&free_b, &total_b));
-    const size_t per_matrix = sizeof(cplx) * ((size_t)L * nh * nh + 4 * MM + (size_t)n_E * 0) + sizeof(double) * (size_t)L * M + sizeof(cplx) * (size_t)M * 64;
-    size_t have = free_b / 2 + p->ld_stash.cap + p->ld_out.cap;
+    Ws &wl = p->ws[0], &wr = p->ws[1];
+    const size_t per_matrix = sizeof(cplx) * (2 * (size_t)L * nh * nh + 4 * MM) + sizeof(double) * (size_t)L * M + sizeof(cplx) * (size_t)M * 256;
+    const size_t held = p->ld_stash.cap + p->ld_stashL.cap + p->ld_out.cap + p->ld_A0.cap + p->ld_A1.cap + wl.G0.cap + wl.G1.cap + wr.G0.cap + wr.G1.cap;
+    const size_t have = free_b / 2 + held;
     int chunk = (int)std::min<size_t>((size_t)batch, std::max<size_t>(1, have / per_matrix));
-    Ws &w = p->ws[0];
-    Buf *four[] = {&p->ld_A0, &p->ld_A1, &p->ld_B0, &p->ld_B1};
-    for (Buf *b : four) if ((rc = ensure(p, *b, sizeof(cplx) * MM * chunk))) return rc;
+    if ((rc = ensure_sweep_ws(p, wl, chunk)) || (rc = ensure_sweep_ws(p, wr, chunk))) return rc;
     if ((rc = ensure(p, p->ld_stash, sizeof(cplx) * (size_t)L * nh * nh * chunk))) return rc;
+    if ((rc = ensure(p, p->ld_stashL, sizeof(cplx) * (size_t)L * nh * nh * chunk))) return rc;
     if ((rc = ensure(p, p->ld_out, sizeof(double) * (size_t)L * M * chunk))) return rc;
-    if ((rc = ensure_inverse_ws(p, w, M, chunk))) return rc;
+    // batches of (matrix, slice) pairs for the G_ii: about 2048 matrices at a time
+    const int ns_max = std::max(1, std::min(L, 2048 / std::max(1, chunk)));
+    const int bmax = ns_max * chunk;
+    if ((rc = ensure(p, p->ld_A0, sizeof(cplx) * MM * bmax)) || (rc = ensure(p, p->ld_A1, sizeof(cplx) * MM * bmax))) return rc;
+    if ((rc = ensure(p, p->ld_B0, sizeof(int) * (size_t)bmax))) return rc;
+    if ((rc = ensure_inverse_ws(p, wl, M, bmax))) return rc;
     p->stats.cohort = chunk;
     const double *E = ptr<double>(p->E);
     const cplx *gLl = ptr<cplx>(p->gL), *gRl = lead_gR(p);
-    cplx *stash = ptr<cplx>(p->ld_stash);
+    cplx *stashR = ptr<cplx>(p->ld_stash), *stashL = ptr<cplx>(p->ld_stashL);
     for (int bz0 = 0; bz0 < batch; bz0 += chunk) {
         const int nb = std::min(chunk, batch - bz0);
         int *status = ptr<int>(p->status) + bz0;
         dim3 ag((unsigned)std::min<size_t>((MM + 255) / 256, 2048), nb), sg((unsigned)std::min((nh * nh + 255) / 256, 1024), nb);
         const size_t sslice = (size_t)nh * nh * nb;          // stash of one slice for the chunk
-        auto assemble = [&](cplx *A, int i, bool left, const cplx *gprev, bool right) {
-            ldos_assemble_kernel<<<ag, 256, 0, p->stream>>>(A, M, L, nh, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
-                                                           ptr<uint8_t>(p->hop), left ? 1 : 0, gprev, gLl, right ? 1 : 0,
-                                                           i + 1 < L ? stash + (size_t)(i + 1) * sslice : nullptr, gRl);
-            p->stats.launches++;
-        };
-        cplx *A0 = ptr<cplx>(p->ld_A0), *A1 = ptr<cplx>(p->ld_A1), *P = ptr<cplx>(p->ld_B0), *Q = ptr<cplx>(p->ld_B1), *res = nullptr;
-        // right-to-left: gR_i, i = L-1 .. 1; slice i - 1 needs its block on S_{i-1}
-        for (int i = L - 1; i >= 1; i--) {
-            assemble(A0, i, false, nullptr, true);
-            if ((rc = run_inverse(p, w, A0, A1, M, nb, status, &res))) return rc;
-            ldos_stash_kernel<<<sg, 256, 0, p->stream>>>(res, stash + (size_t)i * sslice, M, nh, (i - 1) & 1);
-            p->stats.launches++;
-        }
-        // left-to-right: G_ii and gL_i
-        for (int i = 0; i < L; i++) {
-            assemble(A0, i, true, P, true);
-            if (i + 1 < L) assemble(Q, i, true, P, false);
-            if ((rc = run_inverse(p, w, A0, A1, M, nb, status, &res))) return rc;
-            ldos_diag_kernel<<<(nb * M + 255) / 256, 256, 0, p->stream>>>(res, ptr<double>(p->ld_out), status, M, L, i, nb);
-            p->stats.launches++;
-            if (i + 1 < L) {
-                if ((rc = run_inverse(p, w, Q, P, M, nb, status, &res))) return rc;
-                if (res != P) std::swap(P, Q);            // P = gL_i for the next slice
+        // ---- the two chains side by side: gR_i (i = L-1 .. 1) on the second stream, gL_i (i = 0 .. L-2) on the plan's
+        CUDA_TRY(p, cudaEventRecord(p->ev_sync[0], p->stream));
+        CUDA_TRY(p, cudaStreamWaitEvent(wr.stream, p->ev_sync[0], 0));
+        cplx *RA = ptr<cplx>(wr.G0), *RB = ptr<cplx>(wr.G1), *LA = ptr<cplx>(wl.G0), *LB = ptr<cplx>(wl.G1), *Lprev = nullptr, *res = nullptr;
+        for (int s = 0; s < L - 1; s++) {
+            {   // right chain, slice i: A from the stashed block of gR_{i+1} (or the lead)
+                const int i = L - 1 - s;
+                ldos_assemble_kernel<<<ag, 256, 0, wr.stream>>>(RA, M, L, nh, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                               ptr<uint8_t>(p->hop), 0, nullptr, gLl, 1, i + 1 < L ? stashR + (size_t)(i + 1) * sslice : nullptr, gRl);
+                if ((rc = run_inverse(p, wr, RA, RB, M, nb, status, &res))) return rc;
+                ldos_stash_kernel<<<sg, 256, 0, wr.stream>>>(res, stashR + (size_t)i * sslice, M, nh, (i - 1) & 1);
+                p->stats.launches += 2;
             }
+            {   // left chain, slice i: A from the full gL_{i-1} of the previous step (or the lead)
+                const int i = s;
+                cplx *dst = (Lprev == LA) ? LB : LA;
+                ldos_assemble_kernel<<<ag, 256, 0, wl.stream>>>(dst, M, L, nh, i, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite), ptr<uint8_t>(p->bond),
+                                                               ptr<uint8_t>(p->hop), 1, Lprev, gLl, 0, nullptr, gRl);
+                if ((rc = run_inverse(p, wl, dst, dst == LA ? LB : LA, M, nb, status, &res))) return rc;
+                Lprev = res;
+                ldos_stash_kernel<<<sg, 256, 0, wl.stream>>>(res, stashL + (size_t)i * sslice, M, nh, i & 1);
+                p->stats.launches += 2;
+            }
+        }
+        CUDA_TRY(p, cudaGetLastError());
+        CUDA_TRY(p, cudaEventRecord(p->ev_sync[1], wr.stream));
+        CUDA_TRY(p, cudaStreamWaitEvent(p->stream, p->ev_sync[1], 0));
+        // ---- G_ii of all slices: independent, in batches of ns slices x nb matrices
+        int *dstat = ptr<int>(p->ld_B0);
+        for (int i0 = 0; i0 < L; i0 += ns_max) {
+            const int ns = std::min(ns_max, L - i0), nbat = ns * nb;
+            dim3 bg((unsigned)std::min<size_t>((MM + 255) / 256, 64), nbat);
+            ldos_assemble_both_kernel<<<bg, 256, 0, p->stream>>>(ptr<cplx>(p->ld_A0), M, L, nh, i0, nb, n_E, bz0, E, eta, p->t, ptr<double>(p->onsite),
+                                                                ptr<uint8_t>(p->bond), ptr<uint8_t>(p->hop), stashL, stashR, gLl, gRl);
+            CUDA_TRY(p, cudaMemsetAsync(dstat, 0, sizeof(int) * (size_t)nbat, p->stream));
+            if ((rc = run_inverse(p, wl, ptr<cplx>(p->ld_A0), ptr<cplx>(p->ld_A1), M, nbat, dstat, &res))) return rc;
+            const long long tot = (long long)nbat * M;
+            ldos_diag_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, p->stream>>>(res, ptr<double>(p->ld_out), dstat, status, M, L, i0, nb, ns);
+            p->stats.launches += 2;
         }
         CUDA_TRY(p, cudaGetLastError());
         CUDA_TRY(p, cudaMemcpyAsync(ldos_out + (size_t)bz0 * L * M, p->ld_out.p, sizeof(double) * (size_t)L * M * nb, cudaMemcpyDefault, p->stream));
