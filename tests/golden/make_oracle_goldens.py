@@ -5,6 +5,8 @@ CUDA path.  These runs take minutes to an hour of CPU time (naive LU at M = 244 
 why their results are stored instead of being recomputed inside the GPU parity tests.
 
     python tests/golden/make_oracle_goldens.py --config 2 [--threads 8]
+    python tests/golden/make_oracle_goldens.py --config 2 --append 236 246 250 261 266 280
+                                     (more energies of device 0, appended to the stored file; the existing lines stay)
 
 Each output line: dev_index energy_index E[eV] T.  Header lines (#) state the workload recipe.
 Lead self-energies use the oracle's cell form (Sancho-Rubio on the 2M x 2M two-slice cell,
@@ -43,8 +45,11 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--append", type=int, nargs="+", default=None, help="energy indices (device 0) to add to the stored file")
     a = ap.parse_args()
     w, devs, eidx, trunc = subset(a.config)
+    if a.append:
+        devs, eidx = [0], sorted(a.append)
     if trunc:
         w = inputs.truncate(w, trunc)
     E = w.energies[eidx]
@@ -60,6 +65,13 @@ def main():
         for k, e, tk in zip(eidx, E, T):
             lines.append("%d %d %.17g %.17g\n" % (d, k, e, tk))
     dt = time.time() - t0
+    if a.append:
+        with open(out, "a") as f:
+            f.write("# appended by --append %s: same oracle call, %d threads, %.0f s wall\n"
+                    % (" ".join(str(k) for k in eidx), orc.num_threads() if a.threads <= 0 else a.threads, dt))
+            f.writelines(lines)
+        print(out, "appended, %.0f s" % dt)
+        return
     with open(out, "w") as f:
         f.write("# oracle transmissions, written by tests/golden/make_oracle_goldens.py --config %d\n" % a.config)
         f.write("# workload: %s; t=%g eV eta=%g eV; notes=%s; numpy %s\n" % (w.name, w.t, w.eta, w.notes, np.__version__))
