@@ -25,16 +25,103 @@ namespace rgf {
 
 // ------------------------------------------------------------------------------------------
 // Panel factorisation.  blockDim.x = NT, NT * ROWS >= n (thread tid owns rows tid + q NT).  Dynamic shared memory:
-//   pivrow[B] cplx | red_val[32] double | red_idx[32] int | rowAt[n] int | posOf[n] int |
-//   moved[2B] int | nmoved | stage[2B][GJ_CH] cplx
+//   crow[2][NT/32][B] cplx | cinv[2][NT/32] cplx | ckey[2][NT/32] unsigned | rowAt[n] int | posOf[n] int |
+//   moved[2B] int | nmoved
+// The pivot step is the fused kernel's (half_sweep.cuh, hs_pivot_step), widened to NT / 32 candidate warps and B columns:
+// integer search key, every warp's candidate computes its own reciprocal before the one barrier of the step, the pivot row
+// is not a divergent branch.
 // ------------------------------------------------------------------------------------------
-constexpr int GJ_CH = 32;   // columns per chunk when moving exchanged rows
+constexpr int GJ_XPER = 8;  // elements per thread and pass when moving exchanged rows
 
-template <int B>
+template <int B, int NT>
 __host__ __device__ constexpr size_t gj_panel_smem(int n)
 {
-    return sizeof(cplx) * B + sizeof(double) * 32 + sizeof(int) * 32 + sizeof(int) * 2 * (size_t)n +
-           sizeof(int) * (2 * B + 4) + sizeof(cplx) * 2 * B * GJ_CH + 64;
+    return sizeof(cplx) * 2 * (NT / 32) * B + sizeof(cplx) * 2 * (NT / 32) + sizeof(unsigned) * 2 * (NT / 32) +
+           sizeof(int) * 2 * (size_t)n + sizeof(int) * (2 * B + 4) + 64;
+}
+
+struct GJPanelSm {
+    cplx *crow, *cinv;
+    unsigned *ckey;
+    int *rowAt, *posOf;
+};
+
+// One pivot step on column C (static) of the panel.  Key = top 21 bits of max(|re|, |im|) (exponent and 9 mantissa bits: a
+// pivot within 2^-9 of the largest is as good as the largest) | (2047 - row): unique, names the row, lowest row wins ties.
+// Candidate buffers alternate with the parity of C, so one barrier per column suffices.
+//   row[j] <- c + a * pivrow[j]   with (a, c) = (d, 0) on the pivot row and (-x d, row[j]) elsewhere, row[C] <- a.
+template <int C, int B, int NT, int ROWS>
+__device__ __forceinline__ void gj_pivot_step(const GJPanelSm &sm, cplx (&row)[ROWS][B], bool (&used)[ROWS], int k0, int *status_b)
+{
+    constexpr int NW = NT / 32, pb = (C & 1) * NW;
+    static_assert(NW % 4 == 0, "candidate keys are read four at a time");
+    const int tid = threadIdx.x, warp = tid >> 5;
+    unsigned key = 0u;
+    int qs = 0;
+#pragma unroll
+    for (int q = 0; q < ROWS; q++) {
+        const cplx x = row[q][C];
+        const unsigned hre = (unsigned)__double2hiint(x.x) & 0x7fffffffu, him = (unsigned)__double2hiint(x.y) & 0x7fffffffu;
+        const unsigned kq = (used[q] ? 0u : (max(hre, him) & 0xfffff800u)) | (unsigned)(2047 - (tid + q * NT));
+        if (kq > key) { key = kq; qs = q; }
+    }
+    const unsigned wmax = __reduce_max_sync(0xffffffffu, key);
+    if (key == wmax) {
+#pragma unroll
+        for (int q = 0; q < ROWS; q++)
+            if (q == qs) {
+                const cplx x = row[q][C];
+                const double iv = hs_rcp(cabs2(x));
+                sm.ckey[pb + warp] = key;
+                sm.cinv[pb + warp] = cmake(x.x * iv, -x.y * iv);
+#pragma unroll
+                for (int j = 0; j < B; j++) if (j != C) sm.crow[(pb + warp) * B + j] = row[q][j];
+            }
+    }
+    __syncthreads();
+    unsigned best = 0u;
+#pragma unroll
+    for (int w = 0; w < NW; w += 4) {
+        const uint4 k4 = *reinterpret_cast<const uint4 *>(&sm.ckey[pb + w]);
+        best = max(max(best, max(k4.x, k4.y)), max(k4.z, k4.w));
+    }
+    const int pr = 2047 - (int)(best & 0x7ffu), pw = (pr % NT) >> 5;
+    const cplx d = sm.cinv[pb + pw];
+    const cplx *prow = sm.crow + (pb + pw) * B;
+#pragma unroll
+    for (int q = 0; q < ROWS; q++) {
+        const cplx x = row[q][C];
+        const bool is_piv = (tid + q * NT == pr);
+        const cplx nf = cmake(fma(-x.x, d.x, x.y * d.y), fma(-x.x, d.y, -x.y * d.x));     // -(x d)
+        const cplx a = is_piv ? d : nf;
+#pragma unroll
+        for (int j = 0; j < B; j++) {
+            if (j == C) { row[q][j] = a; continue; }
+            const cplx pj = prow[j];
+            cplx c = is_piv ? cmake(0.0, 0.0) : row[q][j];
+            c.x = fma(a.x, pj.x, c.x); c.x = fma(-a.y, pj.y, c.x);
+            c.y = fma(a.x, pj.y, c.y); c.y = fma(a.y, pj.x, c.y);
+            row[q][j] = c;
+        }
+        if (is_piv) {
+            if ((best >> 11) == 0u || best >= 0x7ff00000u) *status_b = 1;          // zero / non-finite pivot
+            used[q] = true;
+            // exchange positions k (= k0 + C) and the position currently holding row pr
+            const int k = k0 + C, ra = sm.rowAt[k], pp = sm.posOf[pr];
+            sm.rowAt[k] = pr; sm.posOf[pr] = k; sm.rowAt[pp] = ra; sm.posOf[ra] = pp;
+        }
+    }
+}
+
+template <int C, int B, int NT, int ROWS>
+__device__ __forceinline__ void gj_pivot_steps(const GJPanelSm &sm, cplx (&row)[ROWS][B], bool (&used)[ROWS], int k0, int bw, int *status_b)
+{
+    if constexpr (C < B) {
+        if (C < bw) {
+            gj_pivot_step<C, B, NT, ROWS>(sm, row, used, k0, status_b);
+            gj_pivot_steps<C + 1, B, NT, ROWS>(sm, row, used, k0, bw, status_b);
+        }
+    }
 }
 
 template <int B, int NT, int ROWS>
@@ -42,22 +129,26 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
                                                       cplx *Nall, cplx *Rall, int *origall, int *status)
 {
     extern __shared__ __align__(16) unsigned char gj_smem[];
-    cplx *pivrow = reinterpret_cast<cplx *>(gj_smem);
-    double *red_val = reinterpret_cast<double *>(pivrow + B);
-    int *red_idx = reinterpret_cast<int *>(red_val + 32);
-    int *rowAt = red_idx + 32;
-    int *posOf = rowAt + n;
+    constexpr int NW = NT / 32;
+    GJPanelSm sm;
+    sm.crow = reinterpret_cast<cplx *>(gj_smem);
+    sm.cinv = sm.crow + 2 * NW * B;
+    sm.ckey = reinterpret_cast<unsigned *>(sm.cinv + 2 * NW);
+    sm.rowAt = reinterpret_cast<int *>(sm.ckey + 2 * NW);
+    sm.posOf = sm.rowAt + n;
+    int *rowAt = sm.rowAt, *posOf = sm.posOf;
     int *moved = posOf + n;
     int *nmoved = moved + 2 * B;
-    cplx *stage = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(nmoved + 4) + 15) & ~(uintptr_t)15);
 
     const int b = blockIdx.x;
     cplx *G = Gall + (long long)b * g_batch;
     cplx *Nbuf = Nall + (long long)b * n * B;
     cplx *Rbuf = Rall + (long long)b * n * B;
     int *orig = origall + (long long)b * n;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x;
     const int bw = (n - k0 < B) ? (n - k0) : B;
+    // 32-byte accesses to the panel columns of a row need (r n + k0) even for every r, and a full panel
+    const bool vec = ((n & 1) == 0) && ((g_batch & 1) == 0) && bw == B && (reinterpret_cast<uintptr_t>(Gall) & 31) == 0;
 
     // thread tid owns rows tid, tid + NT, ... (ROWS of them), each with its B panel entries in registers
     cplx row[ROWS][B];
@@ -65,75 +156,21 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
 #pragma unroll
     for (int q = 0; q < ROWS; q++) {
         const int r = tid + q * NT;
+        if (vec && r < n) {
 #pragma unroll
-        for (int c = 0; c < B; c++) row[q][c] = (r < n && c < bw) ? G[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
+            for (int c = 0; c < B; c += 2)
+                ld256cg(G + (long long)r * n + k0 + c, row[q][c].x, row[q][c].y, row[q][c + 1].x, row[q][c + 1].y);
+        } else {
+#pragma unroll
+            for (int c = 0; c < B; c++) row[q][c] = (r < n && c < bw) ? G[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
+        }
         used[q] = (r >= n || r < k0);     // positions < k0 hold the pivot rows of earlier panels
     }
     for (int i = tid; i < n; i += NT) { rowAt[i] = i; posOf[i] = i; }
+    if (tid < 2 * NW) sm.ckey[tid] = 0u;
     __syncthreads();
 
-    // The column loop is a real loop (an unrolled one is ~400 KB of straight-line code and runs at
-    // instruction-fetch speed); the register-resident row is indexed with select chains instead.
-#pragma unroll 1
-    for (int c = 0; c < bw; c++) {
-        cplx x[ROWS];
-        double v = -1.0;
-        int idx = tid;
-#pragma unroll
-        for (int q = 0; q < ROWS; q++) {
-            x[q] = row[q][0];
-#pragma unroll
-            for (int j = 1; j < B; j++) if (j == c) x[q] = row[q][j];
-            // ---- pivot search: max |x|^2 over unused rows, lowest row index on ties
-            double vq = used[q] ? -1.0 : cabs2(x[q]);
-            if (!(vq == vq)) vq = 1e300;          // NaN: make it win so that it is reported
-            if (vq > v) { v = vq; idx = tid + q * NT; }
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            double ov = __shfl_xor_sync(0xffffffffu, v, off);
-            int oi = __shfl_xor_sync(0xffffffffu, idx, off);
-            if (ov > v || (ov == v && oi < idx)) { v = ov; idx = oi; }
-        }
-        if (lane == 0) { red_val[warp] = v; red_idx[warp] = idx; }
-        __syncthreads();
-        double bv = red_val[0]; int pr = red_idx[0];
-#pragma unroll
-        for (int w = 1; w < NT / 32; w++) {
-            double ov = red_val[w]; int oi = red_idx[w];
-            if (ov > bv || (ov == bv && oi < pr)) { bv = ov; pr = oi; }
-        }
-#pragma unroll
-        for (int q = 0; q < ROWS; q++) {
-            if (tid + q * NT == pr) {
-                if (!(bv > 0.0) || !(bv < 1e299)) status[b] = 1;          // zero / non-finite pivot
-                cplx d = crecip(x[q]);
-#pragma unroll
-                for (int j = 0; j < B; j++) {
-                    cplx y = (j == c) ? cmake(1.0, 0.0) : row[q][j];
-                    row[q][j] = cmul(y, d);
-                    pivrow[j] = row[q][j];
-                }
-                used[q] = true;
-                // exchange positions k (= k0 + c) and the position currently holding row pr
-                int k = k0 + c, a = rowAt[k], pp = posOf[pr];
-                rowAt[k] = pr; posOf[pr] = k; rowAt[pp] = a; posOf[a] = pp;
-            }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < ROWS; q++) {
-            if (tid + q * NT < n && tid + q * NT != pr) {
-#pragma unroll
-                for (int j = 0; j < B; j++) {
-                    cplx y = (j == c) ? cmake(0.0, 0.0) : row[q][j];
-                    cfnma(y, x[q], pivrow[j]);
-                    row[q][j] = y;
-                }
-            }
-        }
-        // pivrow / red_* are rewritten only after the next column's first barrier
-    }
+    gj_pivot_steps<0, B, NT, ROWS>(sm, row, used, k0, bw, status + b);
     __syncthreads();
 
     // ---- list of positions whose row changed
@@ -144,18 +181,29 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     __syncthreads();
     const int nm = *nmoved;                      // <= 2B
 
-    // ---- new panel columns and multipliers (row r now lives at position posOf[r])
+    // ---- new panel columns and multipliers (row r now lives at position posOf[r]); 32-byte stores where aligned
 #pragma unroll
     for (int q = 0; q < ROWS; q++) {
         const int r = tid + q * NT;
         if (r < n) {
             const int pos = posOf[r];
+            if (vec) {
 #pragma unroll
-            for (int c = 0; c < B; c++) {
-                if (c < bw) G[(long long)pos * n + k0 + c] = row[q][c];
-                cplx m = row[q][c];
-                if (pos == k0 + c) m.x -= 1.0;
-                Nbuf[(long long)pos * B + c] = (c < bw) ? m : cmake(0.0, 0.0);
+                for (int c = 0; c < B; c += 2)
+                    st256(G + (long long)pos * n + k0 + c, row[q][c].x, row[q][c].y, row[q][c + 1].x, row[q][c + 1].y);
+            } else {
+#pragma unroll
+                for (int c = 0; c < B; c++)
+                    if (c < bw) G[(long long)pos * n + k0 + c] = row[q][c];
+            }
+#pragma unroll
+            for (int c = 0; c < B; c += 2) {
+                cplx m0 = row[q][c], m1 = row[q][c + 1];
+                if (pos == k0 + c) m0.x -= 1.0;
+                if (pos == k0 + c + 1) m1.x -= 1.0;
+                if (c >= bw) m0 = cmake(0.0, 0.0);
+                if (c + 1 >= bw) m1 = cmake(0.0, 0.0);
+                st256(Nbuf + (long long)pos * B + c, m0.x, m0.y, m1.x, m1.y);
             }
         }
     }
@@ -165,23 +213,47 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     __syncthreads();
     if (tid < nm) orig[moved[tid]] = my_orig;
 
-    // ---- move the exchanged rows in all non-panel columns, chunk by chunk
-    for (int j0 = 0; j0 < n; j0 += GJ_CH) {
-        for (int e = tid; e < nm * GJ_CH; e += NT) {
-            int q = e / GJ_CH, j = j0 + e % GJ_CH;
-            if (j < n && (j < k0 || j >= k0 + B)) stage[q * GJ_CH + (j - j0)] = G[(long long)rowAt[moved[q]] * n + j];
+    // ---- move the exchanged rows in all non-panel columns: passes over disjoint column ranges of cw columns (nm * cw <=
+    // GJ_XPER * NT elements), every element of a pass loaded into registers before any is stored (one barrier per pass; passes
+    // touch different columns, so nothing orders them against each other)
+    if (nm > 0) {
+        const int cw = (GJ_XPER * NT) / nm;
+        for (int j0 = 0; j0 < n; j0 += cw) {
+            const int wj = (n - j0 < cw) ? (n - j0) : cw, cnt = nm * wj;
+            cplx v[GJ_XPER];
+#pragma unroll
+            for (int k = 0; k < GJ_XPER; k++) {
+                const int e = k * NT + tid;
+                if (e < cnt) {
+                    const int q = e / wj, j = j0 + e - q * wj;
+                    if (j < k0 || j >= k0 + B) v[k] = G[(long long)rowAt[moved[q]] * n + j];
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < GJ_XPER; k++) {
+                const int e = k * NT + tid;
+                if (e < cnt) {
+                    const int q = e / wj, j = j0 + e - q * wj;
+                    if (j < k0 || j >= k0 + B) G[(long long)moved[q] * n + j] = v[k];
+                }
+            }
         }
-        __syncthreads();
-        for (int e = tid; e < nm * GJ_CH; e += NT) {
-            int q = e / GJ_CH, j = j0 + e % GJ_CH;
-            if (j < n && (j < k0 || j >= k0 + B)) G[(long long)moved[q] * n + j] = stage[q * GJ_CH + (j - j0)];
-        }
-        __syncthreads();
     }
+    __syncthreads();
     // ---- pivot rows (after the exchange, before the update) for the update kernel
-    for (int e = tid; e < B * n; e += NT) {
-        int c = e / n, j = e % n;
-        Rbuf[(long long)c * n + j] = (c < bw) ? G[(long long)(k0 + c) * n + j] : cmake(0.0, 0.0);
+    for (int e0 = 0; e0 < B * n; e0 += GJ_XPER * NT) {          // GJ_XPER independent loads in flight per thread
+        cplx v[GJ_XPER];
+#pragma unroll
+        for (int k = 0; k < GJ_XPER; k++) {
+            const int e = e0 + k * NT + tid, c = e / n, j = e - c * n;
+            v[k] = (e < B * n && c < bw) ? G[(long long)(k0 + c) * n + j] : cmake(0.0, 0.0);
+        }
+#pragma unroll
+        for (int k = 0; k < GJ_XPER; k++) {
+            const int e = e0 + k * NT + tid;
+            if (e < B * n) Rbuf[e] = v[k];
+        }
     }
 }
 
@@ -192,13 +264,13 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
 // from G and stored back in place (each element is read and written by exactly one lane).
 // 8-column blocks inside the panel [k0, k0+B) are skipped.
 // ------------------------------------------------------------------------------------------
-constexpr int GU_BM = 128, GU_BN = 32, GU_THREADS = 128;
+constexpr int GU_BM = 128, GU_BN = 16, GU_THREADS = 128, GU_NJ = GU_BN / 8;
 template <int B> constexpr int gu_ldn() { return B + 4; }
 constexpr int GU_LDR = GU_BN + 2;
 template <int B> constexpr int gu_smem() { return (GU_BM * gu_ldn<B>() + B * GU_LDR) * (int)sizeof(cplx); }
 
 template <int B>
-__global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long long g_batch, int n, int k0,
+__global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, long long g_batch, int n, int k0,
                                                                const cplx *Nall, const cplx *Rall)
 {
     extern __shared__ __align__(16) unsigned char gu_smem_raw[];
@@ -230,17 +302,26 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
 
     const int wr = row0 + warp * 32;
     int mb_valid = (n - wr + 7) / 8; mb_valid = mb_valid < 0 ? 0 : (mb_valid > 4 ? 4 : mb_valid);
-    int nb_valid = (n - col0 + 7) / 8; nb_valid = nb_valid > 4 ? 4 : nb_valid;
-    bool skipj[4];
+    int nb_valid = (n - col0 + 7) / 8; nb_valid = nb_valid > GU_NJ ? GU_NJ : nb_valid;
+    bool skipj[GU_NJ];
 #pragma unroll
-    for (int j = 0; j < 4; j++) { int c = col0 + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c + 8 <= k0 + B); }
+    for (int j = 0; j < GU_NJ; j++) { int c = col0 + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c + 8 <= k0 + B); }
 
-    double cre[4][4][2], cim[4][4][2];
+    const bool vec = (B % 8 == 0) && ((n & 1) == 0) && ((g_batch & 1) == 0) && (reinterpret_cast<uintptr_t>(Gall) & 31) == 0;
+    double cre[4][GU_NJ][2], cim[4][GU_NJ][2];
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < GU_NJ; j++) {
             int rr = wr + i * 8 + g, c = col0 + j * 8 + 2 * t;
+            if (vec) {
+                // both elements of the lane in one 32-byte access (n even: c < n implies c + 1 < n; B % 8 == 0: a column block is inside
+                // the panel or outside it as a whole)
+                cre[i][j][0] = cim[i][j][0] = cre[i][j][1] = cim[i][j][1] = 0.0;
+                if (i < mb_valid && !skipj[j] && rr < n && c < n)
+                    ld256cg(G + (long long)rr * n + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]);
+                continue;
+            }
 #pragma unroll
             for (int q = 0; q < 2; q++) {
                 cplx v = cmake(0.0, 0.0);
@@ -252,26 +333,27 @@ __global__ void __launch_bounds__(GU_THREADS) gj_update_kernel(cplx *Gall, long 
     const cplx *cA = sN + warp * 32 * LDN;
 #pragma unroll
     for (int kk = 0; kk < B; kk += 4) {
-        cplx a[4], bb[4];
+        cplx a[4], bb[GU_NJ];
 #pragma unroll
         for (int i = 0; i < 4; i++) a[i] = cA[(i * 8 + g) * LDN + kk + t];
 #pragma unroll
-        for (int j = 0; j < 4; j++) bb[j] = sR[(kk + t) * GU_LDR + j * 8 + g];
+        for (int j = 0; j < GU_NJ; j++) bb[j] = sR[(kk + t) * GU_LDR + j * 8 + g];
 #pragma unroll
         for (int i = 0; i < 4; i++)
             if (i < mb_valid) {
                 double nai = -a[i].y;
 #pragma unroll
-                for (int j = 0; j < 4; j++)
+                for (int j = 0; j < GU_NJ; j++)
                     if (!skipj[j]) zmma884(cre[i][j], cim[i][j], a[i].x, a[i].y, nai, bb[j].x, bb[j].y);
             }
     }
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < GU_NJ; j++) {
             int rr = wr + i * 8 + g, c = col0 + j * 8 + 2 * t;
             if (i < mb_valid && !skipj[j] && rr < n) {
+                if (vec) { if (c < n) st256(G + (long long)rr * n + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]); continue; }
 #pragma unroll
                 for (int q = 0; q < 2; q++)
                     if (c + q < n && !(c + q >= k0 && c + q < k0 + B))      // panel columns hold N' already

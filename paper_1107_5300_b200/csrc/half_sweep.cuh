@@ -76,37 +76,6 @@ struct HSTab {
 };
 static_assert(sizeof(HSTab) <= sizeof(cplx) * 2 * (HS_NT / 32) * HS_SB, "HSTab must fit in HSmem::crow");
 
-__device__ __forceinline__ cplx ldcg(const cplx *p)
-{
-    double2 v = __ldcg(reinterpret_cast<const double2 *>(p));
-    return v;
-}
-
-// 32-byte (two complex128) L2 load / store: LDG.E.256 / STG.E.256 on sm_100a; p must be 32-byte aligned
-__device__ __forceinline__ void ld256cg(const cplx *p, double &a, double &b, double &c, double &d)
-{
-    asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
-}
-__device__ __forceinline__ void st256(cplx *p, double a, double b, double c, double d)
-{
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
-
-// 1 / v for v = |x|^2 > 0 on the critical path of every pivot: MUFU.RCP64H seed (20 bits) + two Newton steps
-// (4 dependent DFMAs, ~60 cycles) instead of the IEEE division (~130 cycles on sm_100a).  Relative error
-// ~2e-16, irrelevant for a pivot reciprocal.  v outside the normal range (|x| < 1e-154 or > 1e154) gives 0 / inf /
-// NaN, which the caller reports as a singular pivot through the key check and the propagated non-finite values.
-__device__ __forceinline__ double hs_rcp(double v)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));
-    double e = fma(-v, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-v, r, 1.0);
-    r = fma(r, e, r);
-    return r;
-}
-
 // named barrier over `nthreads` threads (whole warps)
 __device__ __forceinline__ void hs_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 

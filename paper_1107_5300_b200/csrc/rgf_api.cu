@@ -226,7 +226,7 @@ int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status, 
     cplx *Nb = ptr<cplx>(w.Nb), *Rb = ptr<cplx>(w.Rb);
     int *orig = ptr<int>(w.orig);
     for (int k0 = 0; k0 < n; k0 += B) {
-        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B>(n), w.stream>>>(G, gb, n, k0, Nb, Rb, orig, status);
+        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B, NT>(n), w.stream>>>(G, gb, n, k0, Nb, Rb, orig, status);
         p->stats.launches++;
         dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
         gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, gb, n, k0, Nb, Rb);
