@@ -4,19 +4,21 @@
 // (Eq. 4).  Here it is an in-place blocked
 // Gauss-Jordan elimination over panels of B columns, batched over (device, energy):
 //
-//   for each panel K = [k0, k0+B):
-//     gj_panel_kernel  (one CTA per matrix, one thread per row, the row's B panel entries in
+//   for each panel K = [k0, k0+B), ping-pong X -> Y as in gj_inverse32.cuh (rows are never moved):
+//     gj_panel_kernel  (one CTA per matrix, one thread per row of X, the row's B panel entries in
 //                       registers): unblocked Gauss-Jordan with partial pivoting on the n x B
-//                       panel; applies the row exchanges to the whole matrix; leaves
-//                         G[:,K]  = N'        (transformed panel = columns K of the block transform)
-//                         Nbuf    = N' - E_K  (n x B multipliers)
-//                         Rbuf    = G[K,:]    (the B pivot rows before the update)
-//     gj_update_kernel (FP64 tensor cores): G[:,J] += Nbuf * Rbuf[:,J] for all columns J not in K
-//   gj_unpermute_kernel: A^-1[:, orig[pos]] = G[:, pos]  (undo the row exchanges as a column scatter)
+//                       panel; the exchange is the map rowAt[pos] = row of X that belongs at position pos; leaves
+//                         Y[pos,K]   = N'[rowAt[pos],:]  (transformed panel = columns K of the block transform)
+//                         Nbuf[pos,:] = N' - E_K          (n x B multipliers)
+//                         rowAt, orig
+//     gj_update_kernel (FP64 tensor cores): Y[pos,J] = X[rowAt[pos],J] + Nbuf[pos,:] * X[rowAt[k0 + :],J] for all columns J not in K
+//   then X <-> Y;  gj_unpermute_kernel: A^-1[:, orig[pos]] = X[:, pos]  (undo the exchanges as a column scatter)
 //
 // Why this shape: every panel step is the same n x (n-B) x B contraction (no shrinking trailing
 // matrix), all O(n^3) work is DMMA, and the latency-bound pivot search of one matrix overlaps with
-// the panels of the other matrices resident on the SM.
+// the panels of the other matrices resident on the SM.  Round 2: the panel kernel used to exchange the rows physically and
+// to snapshot the pivot rows for the update kernel -- 0.9 MB of traffic per 16-column panel through ONE SM per matrix, at
+// the ~40 GB/s a single SM sustains against DRAM latency; with the ping-pong the update kernel's 2048 CTAs do the gather.
 #pragma once
 #include "rgf_common.cuh"
 #include "zgemm.cuh"
@@ -26,18 +28,16 @@ namespace rgf {
 // ------------------------------------------------------------------------------------------
 // Panel factorisation.  blockDim.x = NT, NT * ROWS >= n (thread tid owns rows tid + q NT).  Dynamic shared memory:
 //   crow[2][NT/32][B] cplx | cinv[2][NT/32] cplx | ckey[2][NT/32] unsigned | rowAt[n] int | posOf[n] int |
-//   moved[2B] int | nmoved
+//   tr[NT/32][32 (B+1) + 8] cplx (per-warp transposition buffer of the epilogue + 32 positions)
 // The pivot step is the fused kernel's (half_sweep.cuh, hs_pivot_step), widened to NT / 32 candidate warps and B columns:
 // integer search key, every warp's candidate computes its own reciprocal before the one barrier of the step, the pivot row
 // is not a divergent branch.
 // ------------------------------------------------------------------------------------------
-constexpr int GJ_XPER = 8;  // elements per thread and pass when moving exchanged rows
-
 template <int B, int NT>
 __host__ __device__ constexpr size_t gj_panel_smem(int n)
 {
     return sizeof(cplx) * 2 * (NT / 32) * B + sizeof(cplx) * 2 * (NT / 32) + sizeof(unsigned) * 2 * (NT / 32) +
-           sizeof(int) * 2 * (size_t)n + sizeof(int) * (2 * B + 4) + 64;
+           sizeof(int) * 2 * (size_t)n + 64 + sizeof(cplx) * (NT / 32) * (32 * (B + 1) + 8);
 }
 
 struct GJPanelSm {
@@ -125,8 +125,8 @@ __device__ __forceinline__ void gj_pivot_steps(const GJPanelSm &sm, cplx (&row)[
 }
 
 template <int B, int NT, int ROWS>
-__global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_batch, int n, int k0,
-                                                      cplx *Nall, cplx *Rall, int *origall, int *status)
+__global__ void __launch_bounds__(NT) gj_panel_kernel(const cplx *Xall, cplx *Yall, long long g_batch, int n, int k0,
+                                                      cplx *Nall, int *rowAtAll, int *origall, int *status)
 {
     extern __shared__ __align__(16) unsigned char gj_smem[];
     constexpr int NW = NT / 32;
@@ -137,18 +137,18 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     sm.rowAt = reinterpret_cast<int *>(sm.ckey + 2 * NW);
     sm.posOf = sm.rowAt + n;
     int *rowAt = sm.rowAt, *posOf = sm.posOf;
-    int *moved = posOf + n;
-    int *nmoved = moved + 2 * B;
+    cplx *tr = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(posOf + n) + 15) & ~(uintptr_t)15);
 
     const int b = blockIdx.x;
-    cplx *G = Gall + (long long)b * g_batch;
+    const cplx *X = Xall + (long long)b * g_batch;
+    cplx *Y = Yall + (long long)b * g_batch;
     cplx *Nbuf = Nall + (long long)b * n * B;
-    cplx *Rbuf = Rall + (long long)b * n * B;
     int *orig = origall + (long long)b * n;
+    int *rowAtG = rowAtAll + (long long)b * n;
     const int tid = threadIdx.x;
     const int bw = (n - k0 < B) ? (n - k0) : B;
     // 32-byte accesses to the panel columns of a row need (r n + k0) even for every r, and a full panel
-    const bool vec = ((n & 1) == 0) && ((g_batch & 1) == 0) && bw == B && (reinterpret_cast<uintptr_t>(Gall) & 31) == 0;
+    const bool vec = ((n & 1) == 0) && ((g_batch & 1) == 0) && bw == B && ((reinterpret_cast<uintptr_t>(Xall) | reinterpret_cast<uintptr_t>(Yall)) & 31) == 0;
 
     // thread tid owns rows tid, tid + NT, ... (ROWS of them), each with its B panel entries in registers
     cplx row[ROWS][B];
@@ -159,10 +159,10 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
         if (vec && r < n) {
 #pragma unroll
             for (int c = 0; c < B; c += 2)
-                ld256cg(G + (long long)r * n + k0 + c, row[q][c].x, row[q][c].y, row[q][c + 1].x, row[q][c + 1].y);
+                ld256cg(X + (long long)r * n + k0 + c, row[q][c].x, row[q][c].y, row[q][c + 1].x, row[q][c + 1].y);
         } else {
 #pragma unroll
-            for (int c = 0; c < B; c++) row[q][c] = (r < n && c < bw) ? G[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
+            for (int c = 0; c < B; c++) row[q][c] = (r < n && c < bw) ? X[(long long)r * n + k0 + c] : cmake(0.0, 0.0);
         }
         used[q] = (r >= n || r < k0);     // positions < k0 hold the pivot rows of earlier panels
     }
@@ -173,96 +173,60 @@ __global__ void __launch_bounds__(NT) gj_panel_kernel(cplx *Gall, long long g_ba
     gj_pivot_steps<0, B, NT, ROWS>(sm, row, used, k0, bw, status + b);
     __syncthreads();
 
-    // ---- list of positions whose row changed
-    if (tid == 0) *nmoved = 0;
-    __syncthreads();
-    for (int i = tid; i < n; i += NT)
-        if (rowAt[i] != i) { int q = atomicAdd(nmoved, 1); moved[q] = i; }
-    __syncthreads();
-    const int nm = *nmoved;                      // <= 2B
-
-    // ---- new panel columns and multipliers (row r now lives at position posOf[r]); 32-byte stores where aligned
+    // ---- new panel columns and multipliers (row r now lives at position posOf[r]).  Full panel, aligned rows: every warp
+    // transposes its 32 rows through shared memory so that a store instruction writes whole 32-byte sectors of 64 / B rows
+    // (B / 2 lanes per row) instead of one sector in each of 32 rows.
 #pragma unroll
     for (int q = 0; q < ROWS; q++) {
         const int r = tid + q * NT;
-        if (r < n) {
+        if (vec) {
+            cplx *tw = tr + (size_t)(tid >> 5) * (32 * (B + 1) + 8);
+            int *pw = reinterpret_cast<int *>(tw + 32 * (B + 1));
+            const int lane = tid & 31;
+#pragma unroll
+            for (int c = 0; c < B; c++) tw[lane * (B + 1) + c] = row[q][c];
+            pw[lane] = r < n ? posOf[r] : -1;
+            __syncwarp();
+            constexpr int LPR = B / 2, RPI = 32 / LPR;          // lanes per row, rows per instruction
+#pragma unroll
+            for (int it = 0; it < 32 / RPI; it++) {
+                const int rr = it * RPI + lane / LPR, c = 2 * (lane % LPR), pos = pw[rr];
+                if (pos >= 0) {
+                    cplx m0 = tw[rr * (B + 1) + c], m1 = tw[rr * (B + 1) + c + 1];
+                    st256(Y + (long long)pos * n + k0 + c, m0.x, m0.y, m1.x, m1.y);
+                    if (pos == k0 + c) m0.x -= 1.0;
+                    if (pos == k0 + c + 1) m1.x -= 1.0;
+                    st256(Nbuf + (long long)pos * B + c, m0.x, m0.y, m1.x, m1.y);
+                }
+            }
+            __syncwarp();
+        } else if (r < n) {
             const int pos = posOf[r];
-            if (vec) {
 #pragma unroll
-                for (int c = 0; c < B; c += 2)
-                    st256(G + (long long)pos * n + k0 + c, row[q][c].x, row[q][c].y, row[q][c + 1].x, row[q][c + 1].y);
-            } else {
-#pragma unroll
-                for (int c = 0; c < B; c++)
-                    if (c < bw) G[(long long)pos * n + k0 + c] = row[q][c];
-            }
-#pragma unroll
-            for (int c = 0; c < B; c += 2) {
-                cplx m0 = row[q][c], m1 = row[q][c + 1];
-                if (pos == k0 + c) m0.x -= 1.0;
-                if (pos == k0 + c + 1) m1.x -= 1.0;
-                if (c >= bw) m0 = cmake(0.0, 0.0);
-                if (c + 1 >= bw) m1 = cmake(0.0, 0.0);
-                st256(Nbuf + (long long)pos * B + c, m0.x, m0.y, m1.x, m1.y);
+            for (int c = 0; c < B; c++) {
+                if (c < bw) Y[(long long)pos * n + k0 + c] = row[q][c];
+                cplx m = row[q][c];
+                if (pos == k0 + c) m.x -= 1.0;
+                Nbuf[(long long)pos * B + c] = (c < bw) ? m : cmake(0.0, 0.0);
             }
         }
     }
-    // ---- origin bookkeeping: orig[pos] <- orig[rowAt[pos]]
-    int my_orig = 0;
-    if (tid < nm) my_orig = orig[rowAt[moved[tid]]];
+    // ---- origin bookkeeping orig[pos] <- orig[rowAt[pos]], and the map for the update kernel
+    int o[ROWS];
+#pragma unroll
+    for (int q = 0; q < ROWS; q++) { const int r = tid + q * NT; o[q] = r < n ? orig[rowAt[r]] : 0; }
     __syncthreads();
-    if (tid < nm) orig[moved[tid]] = my_orig;
-
-    // ---- move the exchanged rows in all non-panel columns: passes over disjoint column ranges of cw columns (nm * cw <=
-    // GJ_XPER * NT elements), every element of a pass loaded into registers before any is stored (one barrier per pass; passes
-    // touch different columns, so nothing orders them against each other)
-    if (nm > 0) {
-        const int cw = (GJ_XPER * NT) / nm;
-        for (int j0 = 0; j0 < n; j0 += cw) {
-            const int wj = (n - j0 < cw) ? (n - j0) : cw, cnt = nm * wj;
-            cplx v[GJ_XPER];
 #pragma unroll
-            for (int k = 0; k < GJ_XPER; k++) {
-                const int e = k * NT + tid;
-                if (e < cnt) {
-                    const int q = e / wj, j = j0 + e - q * wj;
-                    if (j < k0 || j >= k0 + B) v[k] = G[(long long)rowAt[moved[q]] * n + j];
-                }
-            }
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < GJ_XPER; k++) {
-                const int e = k * NT + tid;
-                if (e < cnt) {
-                    const int q = e / wj, j = j0 + e - q * wj;
-                    if (j < k0 || j >= k0 + B) G[(long long)moved[q] * n + j] = v[k];
-                }
-            }
-        }
-    }
-    __syncthreads();
-    // ---- pivot rows (after the exchange, before the update) for the update kernel
-    for (int e0 = 0; e0 < B * n; e0 += GJ_XPER * NT) {          // GJ_XPER independent loads in flight per thread
-        cplx v[GJ_XPER];
-#pragma unroll
-        for (int k = 0; k < GJ_XPER; k++) {
-            const int e = e0 + k * NT + tid, c = e / n, j = e - c * n;
-            v[k] = (e < B * n && c < bw) ? G[(long long)(k0 + c) * n + j] : cmake(0.0, 0.0);
-        }
-#pragma unroll
-        for (int k = 0; k < GJ_XPER; k++) {
-            const int e = e0 + k * NT + tid;
-            if (e < B * n) Rbuf[e] = v[k];
-        }
-    }
+    for (int q = 0; q < ROWS; q++) { const int r = tid + q * NT; if (r < n) { orig[r] = o[q]; rowAtG[r] = rowAt[r]; } }
 }
 
 // ------------------------------------------------------------------------------------------
-// Trailing update on the FP64 tensor pipe: G[:,J] += Nbuf (n x B) * Rbuf[:,J] (B x |J|).
-// CTA = 4 warps stacked on rows: tile 128 rows x 32 columns; the Mult and pivot-row tiles are staged by TMA bulk copies
-// (cp.async.bulk + mbarrier: BASELINE.json north_star "Large M uses TMA-staged panels"); the accumulators are initialised
-// from G and stored back in place (each element is read and written by exactly one lane).
-// 8-column blocks inside the panel [k0, k0+B) are skipped.
+// Trailing update on the FP64 tensor pipe: Y[pos,J] = X[rowAt[pos],J] + Nbuf[pos,:] (n x B) * X[rowAt[k0 + :],J] (B x |J|).
+// CTA = 4 warps stacked on rows: tile 128 rows x 16 columns (rank-16 updates are bound by HBM, not by the tensor pipe: a
+// narrow tile keeps the accumulators at 64 registers so that four CTAs share an SM and their loads overlap); the Mult and
+// pivot-row tiles are staged by TMA bulk copies (cp.async.bulk + mbarrier: BASELINE.json north_star "Large M uses
+// TMA-staged panels"), the pivot rows straight from X through the row map; the accumulators are initialised from X and
+// stored to Y with 32-byte accesses.  8-column blocks inside the panel [k0, k0+B) are skipped.
 // ------------------------------------------------------------------------------------------
 constexpr int GU_BM = 128, GU_BN = 16, GU_THREADS = 128, GU_NJ = GU_BN / 8;
 template <int B> constexpr int gu_ldn() { return B + 4; }
@@ -270,8 +234,8 @@ constexpr int GU_LDR = GU_BN + 2;
 template <int B> constexpr int gu_smem() { return (GU_BM * gu_ldn<B>() + B * GU_LDR) * (int)sizeof(cplx); }
 
 template <int B>
-__global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, long long g_batch, int n, int k0,
-                                                               const cplx *Nall, const cplx *Rall)
+__global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(const cplx *Xall, cplx *Yall, long long g_batch, int n, int k0,
+                                                               const cplx *Nall, const int *rowAtAll)
 {
     extern __shared__ __align__(16) unsigned char gu_smem_raw[];
     cplx *sN = reinterpret_cast<cplx *>(gu_smem_raw);
@@ -279,9 +243,10 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, lo
     constexpr int LDN = gu_ldn<B>();
 
     const int b = blockIdx.z;
-    cplx *G = Gall + (long long)b * g_batch;
+    const cplx *X = Xall + (long long)b * g_batch;
+    cplx *Y = Yall + (long long)b * g_batch;
     const cplx *Nbuf = Nall + (long long)b * n * B;
-    const cplx *Rbuf = Rall + (long long)b * n * B;
+    const int *rowAt = rowAtAll + (long long)b * n;
     const int row0 = blockIdx.y * GU_BM, col0 = blockIdx.x * GU_BN;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     // whole tile inside the panel: nothing to do
@@ -291,14 +256,19 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, lo
     // stage Mult (rows row0 .., B columns: one contiguous row of the panel buffer each) and the B pivot rows (32 columns
     // from col0) with TMA bulk copies; rows / columns beyond n are not loaded (they only feed accumulators that are never stored)
     __shared__ unsigned long long bar;
+    __shared__ int sRowM[GU_BM];          // rows of X that belong at positions row0 .. row0 + 127
     const int nrows = (n - row0 < GU_BM) ? (n - row0) : GU_BM, ncolsR = (n - col0 < GU_BN) ? (n - col0) : GU_BN;
+    const int bw = (n - k0 < B) ? (n - k0) : B;
     if (tid == 0) tma_bar_init(&bar, 1);
+    for (int rr = tid; rr < GU_BM; rr += GU_THREADS) sRowM[rr] = rr < nrows ? rowAt[row0 + rr] : 0;
+    // pivot rows beyond a narrow last panel: zero (their Mult columns are zero, but shared memory may hold NaN patterns)
+    for (int e = tid; e < (B - bw) * GU_BN; e += GU_THREADS) sR[(bw + e / GU_BN) * GU_LDR + e % GU_BN] = cmake(0.0, 0.0);
     __syncthreads();
-    if (tid == 0) tma_expect(&bar, (unsigned)(nrows * B + B * ncolsR) * (unsigned)sizeof(cplx));
+    if (tid == 0) tma_expect(&bar, (unsigned)(nrows * B + bw * ncolsR) * (unsigned)sizeof(cplx));
     for (int rr = tid; rr < nrows; rr += GU_THREADS)
         tma_load_row(sN + rr * LDN, Nbuf + (long long)(row0 + rr) * B, B * (unsigned)sizeof(cplx), &bar);
-    for (int k = tid; k < B; k += GU_THREADS)
-        tma_load_row(sR + k * GU_LDR, Rbuf + (long long)k * n + col0, ncolsR * (unsigned)sizeof(cplx), &bar);
+    for (int k = tid; k < bw; k += GU_THREADS)
+        tma_load_row(sR + k * GU_LDR, X + (long long)rowAt[k0 + k] * n + col0, ncolsR * (unsigned)sizeof(cplx), &bar);
 
     const int wr = row0 + warp * 32;
     int mb_valid = (n - wr + 7) / 8; mb_valid = mb_valid < 0 ? 0 : (mb_valid > 4 ? 4 : mb_valid);
@@ -307,25 +277,26 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, lo
 #pragma unroll
     for (int j = 0; j < GU_NJ; j++) { int c = col0 + j * 8; skipj[j] = (j >= nb_valid) || (c >= k0 && c + 8 <= k0 + B); }
 
-    const bool vec = (B % 8 == 0) && ((n & 1) == 0) && ((g_batch & 1) == 0) && (reinterpret_cast<uintptr_t>(Gall) & 31) == 0;
+    const bool vec = (B % 8 == 0) && ((n & 1) == 0) && ((g_batch & 1) == 0) && ((reinterpret_cast<uintptr_t>(Xall) | reinterpret_cast<uintptr_t>(Yall)) & 31) == 0;
     double cre[4][GU_NJ][2], cim[4][GU_NJ][2];
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < GU_NJ; j++) {
             int rr = wr + i * 8 + g, c = col0 + j * 8 + 2 * t;
+            const cplx *src = X + (long long)((i < mb_valid && rr < n) ? sRowM[rr - row0] : 0) * n;
             if (vec) {
                 // both elements of the lane in one 32-byte access (n even: c < n implies c + 1 < n; B % 8 == 0: a column block is inside
                 // the panel or outside it as a whole)
                 cre[i][j][0] = cim[i][j][0] = cre[i][j][1] = cim[i][j][1] = 0.0;
                 if (i < mb_valid && !skipj[j] && rr < n && c < n)
-                    ld256cg(G + (long long)rr * n + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]);
+                    ld256cg(src + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]);
                 continue;
             }
 #pragma unroll
             for (int q = 0; q < 2; q++) {
                 cplx v = cmake(0.0, 0.0);
-                if (i < mb_valid && !skipj[j] && rr < n && c + q < n) v = G[(long long)rr * n + c + q];
+                if (i < mb_valid && !skipj[j] && rr < n && c + q < n) v = src[c + q];
                 cre[i][j][q] = v.x; cim[i][j][q] = v.y;
             }
         }
@@ -353,11 +324,11 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(cplx *Gall, lo
         for (int j = 0; j < GU_NJ; j++) {
             int rr = wr + i * 8 + g, c = col0 + j * 8 + 2 * t;
             if (i < mb_valid && !skipj[j] && rr < n) {
-                if (vec) { if (c < n) st256(G + (long long)rr * n + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]); continue; }
+                if (vec) { if (c < n) st256(Y + (long long)rr * n + c, cre[i][j][0], cim[i][j][0], cre[i][j][1], cim[i][j][1]); continue; }
 #pragma unroll
                 for (int q = 0; q < 2; q++)
                     if (c + q < n && !(c + q >= k0 && c + q < k0 + B))      // panel columns hold N' already
-                        G[(long long)rr * n + c + q] = cmake(cre[i][j][q], cim[i][j][q]);
+                        Y[(long long)rr * n + c + q] = cmake(cre[i][j][q], cim[i][j][q]);
             }
         }
 }

@@ -136,6 +136,9 @@ int set_kernel_attrs(rgf_plan *p)
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<16>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<8>()));
     CUDA_TRY(p, cudaFuncSetAttribute(gj_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gu_smem<4>()));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_panel_kernel<16, 512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj_panel_smem<16, 512>(512)));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_panel_kernel<8, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj_panel_smem<8, 1024>(1024)));
+    CUDA_TRY(p, cudaFuncSetAttribute(gj_panel_kernel<4, 1024, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj_panel_smem<4, 1024>(2048)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gj32_panel_smem(256)));
     CUDA_TRY(p, cudaFuncSetAttribute(gj32_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GU32_SMEM));
     CUDA_TRY(p, cudaFuncSetAttribute(half_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HSmem)));
@@ -213,36 +216,38 @@ int ensure_inverse_ws(rgf_plan *p, Ws &w, int n, int batch)
 {
     int B = panel_width(n), rc;
     if ((rc = ensure(p, w.Nb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
-    if (n > 256 && (rc = ensure(p, w.Rb, sizeof(cplx) * (size_t)n * B * batch))) return rc;
     if ((rc = ensure(p, w.rowAt, sizeof(int) * (size_t)n * batch))) return rc;
     if ((rc = ensure(p, w.orig, sizeof(int) * (size_t)n * batch))) return rc;
     return RGF_OK;
 }
 
-// generic in-place path (256 < n <= 1024): panels of 16 or 8 columns, physical row exchanges
+// generic path (256 < n <= 2048): panels of 16, 8 or 4 columns, ping-pong X -> Y (rows never move); *result = buffer with the inverse
 template <int B, int NT, int ROWS>
-int inverse_inplace(rgf_plan *p, Ws &w, cplx *G, int n, int batch, int *status, long long gb)
+int inverse_generic(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, long long gb, cplx **result)
 {
-    cplx *Nb = ptr<cplx>(w.Nb), *Rb = ptr<cplx>(w.Rb);
-    int *orig = ptr<int>(w.orig);
+    cplx *Nb = ptr<cplx>(w.Nb);
+    int *orig = ptr<int>(w.orig), *rowAt = ptr<int>(w.rowAt);
+    cplx *X = G, *Y = Galt;
     for (int k0 = 0; k0 < n; k0 += B) {
-        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B, NT>(n), w.stream>>>(G, gb, n, k0, Nb, Rb, orig, status);
+        gj_panel_kernel<B, NT, ROWS><<<batch, NT, gj_panel_smem<B, NT>(n), w.stream>>>(X, Y, gb, n, k0, Nb, rowAt, orig, status);
         p->stats.launches++;
         dim3 grid((n + GU_BN - 1) / GU_BN, (n + GU_BM - 1) / GU_BM, batch);
-        gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(G, gb, n, k0, Nb, Rb);
+        gj_update_kernel<B><<<grid, GU_THREADS, gu_smem<B>(), w.stream>>>(X, Y, gb, n, k0, Nb, rowAt);
         p->stats.launches++;
         CUDA_TRY(p, cudaGetLastError());
+        std::swap(X, Y);
     }
     int nw = n > 512 ? 4 : 8;
     dim3 grid((n + nw - 1) / nw, batch);
-    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), w.stream>>>(G, gb, n, orig);
+    gj_unpermute_kernel<<<grid, nw * 32, (size_t)nw * n * sizeof(cplx), w.stream>>>(X, gb, n, orig);
     p->stats.launches++;
     CUDA_TRY(p, cudaGetLastError());
+    *result = X;
     return RGF_OK;
 }
 
 // Inverse of `batch` n x n matrices stored at G (stride n*n).  Galt is a second buffer of the same
-// size; *result is G or Galt, whichever holds the inverse (n <= 256 ping-pongs between the two).
+// size; *result is G or Galt, whichever holds the inverse (every path ping-pongs between the two).
 // status[b] is set to 1 on a zero / non-finite pivot.
 int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *status, cplx **result, long long stride = 0)
 {
@@ -252,9 +257,9 @@ int run_inverse(rgf_plan *p, Ws &w, cplx *G, cplx *Galt, int n, int batch, int *
     const int total = n * batch;
     gj_init_orig_kernel<<<(total + 255) / 256, 256, 0, w.stream>>>(orig, n, total);
     p->stats.launches++;
-    if (n > 1024) { *result = G; return inverse_inplace<4, 1024, 2>(p, w, G, n, batch, status, gb); }
-    if (n > 512) { *result = G; return inverse_inplace<8, 1024, 1>(p, w, G, n, batch, status, gb); }
-    if (n > 256) { *result = G; return inverse_inplace<16, 512, 1>(p, w, G, n, batch, status, gb); }
+    if (n > 1024) return inverse_generic<4, 1024, 2>(p, w, G, Galt, n, batch, status, gb, result);
+    if (n > 512) return inverse_generic<8, 1024, 1>(p, w, G, Galt, n, batch, status, gb, result);
+    if (n > 256) return inverse_generic<16, 512, 1>(p, w, G, Galt, n, batch, status, gb, result);
     cplx *X = G, *Y = Galt, *Mult = ptr<cplx>(w.Nb);
     int *rowAt = ptr<int>(w.rowAt);
     for (int k0 = 0; k0 < n; k0 += G32_B) {
@@ -326,7 +331,7 @@ int run_lead_side(rgf_plan *p, int n_E, double eta, int side, int pa, int pb, bo
     Buf *cb[] = {&p->l_alpha, &p->l_beta, &p->l_T1, &p->l_T2, &p->l_T3, &p->l_eps, &p->l_eps_s, &p->stage_in};
     for (Buf *b : cb) if ((rc = ensure(p, *b, sizeof(cplx) * CC * n_E))) return rc;
     if ((rc = ensure(p, p->l_W, sizeof(cplx) * NN * n_E))) return rc;
-    if (N <= 256 && (rc = ensure(p, p->l_W2, sizeof(cplx) * NN * n_E))) return rc;
+    if ((rc = ensure(p, p->l_W2, sizeof(cplx) * NN * n_E))) return rc;
     if ((rc = ensure_inverse_ws(p, w, N, n_E))) return rc;
     cplx *a = ptr<cplx>(p->l_alpha), *b = ptr<cplx>(p->l_beta), *X = ptr<cplx>(p->l_eps), *Y = ptr<cplx>(p->l_eps_s);
     cplx *T1 = ptr<cplx>(p->l_T1), *T2 = ptr<cplx>(p->l_T2), *an = ptr<cplx>(p->l_T3);
