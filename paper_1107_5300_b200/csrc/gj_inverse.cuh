@@ -256,11 +256,12 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(const cplx *Xa
     // stage Mult (rows row0 .., B columns: one contiguous row of the panel buffer each) and the B pivot rows (32 columns
     // from col0) with TMA bulk copies; rows / columns beyond n are not loaded (they only feed accumulators that are never stored)
     __shared__ unsigned long long bar;
-    __shared__ int sRowM[GU_BM];          // rows of X that belong at positions row0 .. row0 + 127
+    __shared__ int sRowM[GU_BM], sRowK[B];          // rows of X that belong at positions row0 .. row0 + 127 and k0 .. k0 + B - 1
     const int nrows = (n - row0 < GU_BM) ? (n - row0) : GU_BM, ncolsR = (n - col0 < GU_BN) ? (n - col0) : GU_BN;
     const int bw = (n - k0 < B) ? (n - k0) : B;
     if (tid == 0) tma_bar_init(&bar, 1);
     for (int rr = tid; rr < GU_BM; rr += GU_THREADS) sRowM[rr] = rr < nrows ? rowAt[row0 + rr] : 0;
+    if (tid >= GU_THREADS - B) { const int k = tid - (GU_THREADS - B); sRowK[k] = k < bw ? rowAt[k0 + k] : 0; }
     // pivot rows beyond a narrow last panel: zero (their Mult columns are zero, but shared memory may hold NaN patterns)
     for (int e = tid; e < (B - bw) * GU_BN; e += GU_THREADS) sR[(bw + e / GU_BN) * GU_LDR + e % GU_BN] = cmake(0.0, 0.0);
     __syncthreads();
@@ -268,7 +269,7 @@ __global__ void __launch_bounds__(GU_THREADS, 4) gj_update_kernel(const cplx *Xa
     for (int rr = tid; rr < nrows; rr += GU_THREADS)
         tma_load_row(sN + rr * LDN, Nbuf + (long long)(row0 + rr) * B, B * (unsigned)sizeof(cplx), &bar);
     for (int k = tid; k < bw; k += GU_THREADS)
-        tma_load_row(sR + k * GU_LDR, X + (long long)rowAt[k0 + k] * n + col0, ncolsR * (unsigned)sizeof(cplx), &bar);
+        tma_load_row(sR + k * GU_LDR, X + (long long)sRowK[k] * n + col0, ncolsR * (unsigned)sizeof(cplx), &bar);
 
     const int wr = row0 + warp * 32;
     int mb_valid = (n - wr + 7) / 8; mb_valid = mb_valid < 0 ? 0 : (mb_valid > 4 ? 4 : mb_valid);
