@@ -46,7 +46,7 @@ struct Buf {
 struct Ws {
     cudaStream_t stream = nullptr;
     bool own_stream = false;
-    Buf G0, G1, Nb, Rb, rowAt, orig, Pa, Pb;
+    Buf G0, G1, Nb, rowAt, orig, Pa, Pb;
     Buf H0, H1, H2, Wc, Tr, Fx0, Fx1, Fp0, Fp1, Fperm, Cp0, Cp1;                        // half-slice formulation: three compact g buffers, C P, trace scratch
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> upd_events;
     size_t upd_used = 0;
@@ -1139,7 +1139,7 @@ int rgf_destroy(rgf_plan *p)
     for (Buf *b : bufs) release(*b);
     for (Ws &w : p->ws) {
         if (w.stream) cudaStreamSynchronize(w.stream);
-        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.Rb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm, &w.Cp0, &w.Cp1};
+        Buf *wb[] = {&w.G0, &w.G1, &w.Nb, &w.rowAt, &w.orig, &w.Pa, &w.Pb, &w.H0, &w.H1, &w.H2, &w.Wc, &w.Tr, &w.Fx0, &w.Fx1, &w.Fp0, &w.Fp1, &w.Fperm, &w.Cp0, &w.Cp1};
         for (Buf *b : wb) release(*b);
         for (auto &pr : w.upd_events) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
         if (w.own_stream && w.stream) cudaStreamDestroy(w.stream);
