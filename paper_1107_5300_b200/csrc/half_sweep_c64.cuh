@@ -12,19 +12,22 @@
 // is float.  TF32 tensor cores are not used: their 10-bit mantissa cannot hold 1e-3 over thousands of slices.
 //
 // One CTA (512 threads) owns one (device, energy) pair for the whole sweep.  The n x n matrix of a half-step
-// lives in REGISTERS during the elimination (thread (w, l) = (warp, lane) owns rows w + 16 i, columns l + 32 j:
-// 8 x 4 elements), g of the previous half-step in shared memory, only the propagator streams through L2:
+// lives in REGISTERS during the elimination: four threads per row (r = tid / 4, q = tid % 4), thread q holding the working
+// columns 4 s + q, s = 0..31, in 32 register slots.  The column being eliminated always sits in slot 0 (static register
+// index: no select chains, no spills): after the four pivots of a group the slots rotate by one.  g of the previous half-step
+// lives in shared memory, only the propagator streams through L2:
 //     assembly   A <- z - eps - C g_prev C^T [- Sigma]          registers <- shared memory
-//     inverse    unblocked Gauss-Jordan with partial pivoting (rows never move), 2 barriers per pivot
+//     inverse    unblocked Gauss-Jordan with partial pivoting (rows never move): integer key + REDUX search, the row's
+//                multiplier by a shuffle inside its four threads, 2 barriers per pivot
 //     g          scattered to shared memory in true order       g[k][p_c] = X[p_k][c]
-//     propagator P <- g (C P_prev), 32-column tiles of C P_prev staged in shared memory, FFMA register tiles
+//     propagator P <- g (C P_prev), 64-column tiles of C P_prev staged in shared memory, FFMA register tiles (8 rows x 2 columns)
 #pragma once
 #include "half_kernels.cuh"
 #include "rgf_common.cuh"
 
 namespace rgf {
 
-constexpr int HC_NT = 512, HC_NMAX = 128, HC_LDG = HC_NMAX + 1, HC_LDW = 33;
+constexpr int HC_NT = 512, HC_NMAX = 128, HC_LDG = HC_NMAX + 1, HC_TW = 64, HC_LDW = HC_TW + 2;
 
 struct HC64Args {
     int M, L, nh, n_E, bz0, nb;
@@ -40,12 +43,12 @@ struct HC64Args {
 
 struct HC64Smem {
     float2 g[HC_NMAX * HC_LDG];       // g of the previous half-step, true order
-    float2 Wt[HC_NMAX * HC_LDW];      // tile of C P_prev
-    float2 colk[2][HC_NMAX], prow[2][HC_NMAX];
+    alignas(16) float2 Wt[HC_NMAX * HC_LDW];      // tile of C P_prev (64 columns)
+    alignas(16) float2 prow[4 * 34];  // pivot row as it stands (unscaled), thread q's 32 slots at prow[34 q + s] (34: LDS.128 conflict-free)
+    alignas(16) unsigned wkey[HC_NT / 32];   // per-warp maximum of the search key (read four at a time)
     float eps_re[HC_NMAX];            // E - eps_j, formed in double, rounded
     short ra[HC_NMAX], rb[HC_NMAX];   // kind B: ra = m'; kind F: lower / upper B neighbour (or -1)
     int perm[HC_NMAX], pinv[HC_NMAX];
-    unsigned char used[HC_NMAX];
 };
 
 __device__ __forceinline__ float2 c64mul(float2 a, float2 b) { return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x)); }
@@ -63,7 +66,8 @@ __global__ void __launch_bounds__(HC_NT, 1) half_sweep_c64_kernel(HC64Args a)
     float2 *Pb[2] = {a.P0 + (long long)bl * HC_NMAX * HC_NMAX, a.P1 + (long long)bl * HC_NMAX * HC_NMAX};
     const cplx *gl = a.gL + (long long)e * MM, *gr = a.gR + (long long)e * MM;
     int n = 0;
-    float2 X[8][4];
+    const int rr_ = tid >> 2, q = tid & 3, lane = l;       // row of this thread, its column residue, lane
+    float2 X[32];
 
     for (int hs = 0; hs < a.hs_end; hs++) {
         const int i = hs >> 1, kind = hs & 1, cur = hs & 1;
@@ -80,26 +84,37 @@ __global__ void __launch_bounds__(HC_NT, 1) half_sweep_c64_kernel(HC64Args a)
             sm.eps_re[r] = (float)((E - eps[2 * r + par]) / a.t);
             if (kind == 0) { sm.ra[r] = mk[2 * r + par] ? 1 : 0; sm.rb[r] = -1; }
             else { sm.ra[r] = (short)half_nbr(r, par, 0, M, hp); sm.rb[r] = (short)half_nbr(r, par, 1, M, hp); }
-            sm.used[r] = 0;
         }
         __syncthreads();
-        // ---- assembly into registers ----
+        // Columns are eliminated in a rotated order that changes from half-step to half-step: working column c' is true
+        // column (c' + shift) mod n.  In a clean ribbon every slice repeats the same arithmetic on the same numbers, so the
+        // rounding errors of a fixed elimination order repeat too and add up coherently: an effective gain or loss per slice,
+        // |dT| growing linearly with L (measured on the clean configs[3] ribbon: median 3.0e-4, maximum 1.5e-3 at L = 2000,
+        // ten times the disordered ribbon's; carrying the propagator in double or symmetrising g changed nothing).  A
+        // different order per half-step gives the same inverse with different roundings, and the errors add like a random
+        // walk instead (median 6e-5, maximum 3.2e-4).
+        const int shift = (int)(((unsigned)hs * 2654435761u >> 8) % (unsigned)n);
+        // ---- assembly into registers: slot s <- A[r][(4 s + q + shift) mod n] ----
+        {
+            const int r = rr_;
+            const bool rok = r < n;
+            const int ua = rok ? sm.ra[r] : -1, ub = rok ? sm.rb[r] : -1;
+            const float er = rok ? sm.eps_re[r] : 0.f;
 #pragma unroll
-        for (int ii = 0; ii < 8; ii++)
-#pragma unroll
-            for (int jj = 0; jj < 4; jj++) {
-                const int r = w + 16 * ii, c = l + 32 * jj;
+            for (int sl = 0; sl < 32; sl++) {
+                const int cw = 4 * sl + q;
+                int c = cw + shift; if (c >= n) c -= n;
                 float2 v = make_float2(0.f, 0.f);
-                if (r < n && c < n) {
-                    if (r == c) v = make_float2(sm.eps_re[r], etaf);
+                if (rok && cw < n) {
+                    if (r == c) v = make_float2(er, etaf);
                     float sx = 0.f, sy = 0.f;
                     if (kind == 0) {
-                        if (sm.ra[r] && sm.ra[c]) {
+                        if (ua && sm.ra[c]) {
                             if (first) { const cplx gg = gl[(long long)(2 * r + par) * M + 2 * c + par]; sx = (float)(a.t * gg.x); sy = (float)(a.t * gg.y); }
                             else { const float2 gg = sm.g[r * HC_LDG + c]; sx = gg.x; sy = gg.y; }
                         }
                     } else {
-                        const int ua = sm.ra[r], ub = sm.rb[r], ca = sm.ra[c], cb = sm.rb[c];
+                        const int ca = sm.ra[c], cb = sm.rb[c];
                         if (ua >= 0) {
                             if (ca >= 0) { const float2 gg = sm.g[ua * HC_LDG + ca]; sx += gg.x; sy += gg.y; }
                             if (cb >= 0) { const float2 gg = sm.g[ua * HC_LDG + cb]; sx += gg.x; sy += gg.y; }
@@ -116,101 +131,109 @@ __global__ void __launch_bounds__(HC_NT, 1) half_sweep_c64_kernel(HC64Args a)
                         if (mr[jr] && mr[jc]) { const cplx gg = gr[(long long)jr * M + jc]; v.x -= (float)(a.t * gg.x); v.y -= (float)(a.t * gg.y); }
                     }
                 }
-                X[ii][jj] = v;
+                X[sl] = v;
             }
+        }
         __syncthreads();          // everybody has read g_prev
         // ---- Gauss-Jordan with partial pivoting in registers ----
-        // Columns are eliminated in a rotated order that changes from half-step to half-step.  In a clean ribbon every slice
-        // repeats the same arithmetic on the same numbers, so the rounding errors of a fixed elimination order repeat too
-        // and add up coherently: an effective gain or loss per slice, |dT| growing linearly with L (measured on the clean
-        // configs[3] ribbon: median 3.0e-4, maximum 1.5e-3 at L = 2000, ten times the disordered ribbon's; carrying the
-        // propagator in double or symmetrising g changed nothing).  A different order per half-step gives the same inverse
-        // with different roundings, and the errors add like a random walk instead (median 6e-5, maximum 3.2e-4).
-        const int shift = (int)(((unsigned)hs * 2654435761u >> 8) % (unsigned)n);
-        for (int step = 0; step < n; step++) {
-            const int k = (step + shift < n) ? step + shift : step + shift - n;
-            const int kb = step & 1, jk = k >> 5;
-            if (l == (k & 31)) {
+        bool used = !(rr_ < n);
+        const int ngroups = (n + 3) >> 2;
+#pragma unroll 1
+        for (int g4 = 0; g4 < ngroups; g4++) {
 #pragma unroll
-                for (int ii = 0; ii < 8; ii++) {
-                    float2 v = X[ii][0];
+            for (int qq = 0; qq < 4; qq++) {
+                const int cw = 4 * g4 + qq;                 // working column of this step, in slot 0 of the threads q == qq
+                if (cw < n) {
+                    int k = cw + shift; if (k >= n) k -= n;
+                    // search key: top 25 bits of max(|re|, |im|) | (127 - row): unique, names the row, lowest row wins ties
+                    const float2 x0 = X[0];
+                    const unsigned ure = __float_as_uint(x0.x) & 0x7fffffffu, uim = __float_as_uint(x0.y) & 0x7fffffffu;
+                    unsigned key = 0u;
+                    if (q == qq) key = (used ? 0u : (max(ure, uim) & 0xffffff80u)) | (unsigned)(127 - rr_);
+                    const unsigned wmax = __reduce_max_sync(0xffffffffu, key);
+                    if (lane == 0) sm.wkey[w] = wmax;
+                    // the row's multiplier (its entry in the working column) for all four threads of the row
+                    float2 xr;
+                    xr.x = __shfl_sync(0xffffffffu, x0.x, (lane & ~3) | qq);
+                    xr.y = __shfl_sync(0xffffffffu, x0.y, (lane & ~3) | qq);
+                    __syncthreads();
+                    unsigned best = 0u;
 #pragma unroll
-                    for (int jj = 1; jj < 4; jj++) if (jj == jk) v = X[ii][jj];
-                    sm.colk[kb][w + 16 * ii] = v;
+                    for (int ww = 0; ww < HC_NT / 32; ww += 4) {
+                        const uint4 k4 = *reinterpret_cast<const uint4 *>(&sm.wkey[ww]);
+                        best = max(max(best, max(k4.x, k4.y)), max(k4.z, k4.w));
+                    }
+                    const int p = 127 - (int)(best & 127u);
+                    const bool is_piv = (rr_ == p);
+                    if (is_piv) {
+                        // the pivot row publishes itself as it stands; every row scales its own multiplier instead (f = x_r / pivot)
+                        float4 *dst = reinterpret_cast<float4 *>(sm.prow + 34 * q);
+#pragma unroll
+                        for (int sl = 0; sl < 32; sl += 2) dst[sl >> 1] = make_float4(X[sl].x, X[sl].y, X[sl + 1].x, X[sl + 1].y);
+                        if (q == qq) {
+                            if ((best >> 7) == 0u || best >= 0x7f800000u) a.status[bl] = 1;       // zero / non-finite pivot
+                            sm.perm[k] = p; sm.pinv[p] = k;
+                        }
+                        used = true;
+                    }
+                    // 1 / pivot from the pivot element, which every thread of the CTA can read after the barrier
+                    __syncthreads();
+                    const float2 xp = sm.prow[34 * qq];                  // slot 0 of thread qq of the pivot row = the pivot element
+                    const float m2 = fmaf(xp.x, xp.x, xp.y * xp.y);
+                    const float inv = 1.0f / m2;
+                    const float2 dd = make_float2(xp.x * inv, -xp.y * inv);
+                    const float2 f = c64mul(xr, dd);                     // multiplier of the unscaled pivot row
+                    const float4 *prq = reinterpret_cast<const float4 *>(sm.prow + 34 * q);
+                    if ((p >> 3) != w) {
+                        // no row of this warp is the pivot row (15 warps of 16): v <- v - f * prow, nothing to select
+#pragma unroll
+                        for (int sl = 0; sl < 32; sl += 2) {
+                            const float4 pr = prq[sl >> 1];
+                            float2 v = X[sl], u = X[sl + 1];
+                            v.x = fmaf(-f.x, pr.x, v.x); v.x = fmaf(f.y, pr.y, v.x); v.y = fmaf(-f.x, pr.y, v.y); v.y = fmaf(-f.y, pr.x, v.y);
+                            u.x = fmaf(-f.x, pr.z, u.x); u.x = fmaf(f.y, pr.w, u.x); u.y = fmaf(-f.x, pr.w, u.y); u.y = fmaf(-f.y, pr.z, u.y);
+                            X[sl] = v; X[sl + 1] = u;
+                        }
+                        if (q == qq) X[0] = make_float2(-f.x, -f.y);
+                    } else {
+#pragma unroll
+                        for (int sl = 0; sl < 32; sl++) {
+                            const float2 pr = sm.prow[34 * q + sl];
+                            float2 v = X[sl];
+                            if (sl == 0 && q == qq) v = is_piv ? dd : make_float2(-f.x, -f.y);
+                            else if (is_piv) v = c64mul(pr, dd);
+                            else { v.x = fmaf(-f.x, pr.x, v.x); v.x = fmaf(f.y, pr.y, v.x); v.y = fmaf(-f.x, pr.y, v.y); v.y = fmaf(-f.y, pr.x, v.y); }
+                            X[sl] = v;
+                        }
+                    }
                 }
             }
-            __syncthreads();
-            // every warp finds the pivot itself (same data, same answer): lane handles rows l, l+32, l+64, l+96
-            float best = -1.f; int brow = 0;
+            // rotate the slots: the next group's working columns move into slot 0
+            const float2 x0 = X[0];
 #pragma unroll
-            for (int q = 0; q < 4; q++) {
-                const int r = l + 32 * q;
-                if (r < n && !sm.used[r]) {
-                    const float2 v = sm.colk[kb][r];
-                    float m2 = fmaf(v.x, v.x, v.y * v.y);
-                    if (!(m2 == m2)) m2 = 3.0e38f;            // NaN: report it
-                    if (m2 > best) { best = m2; brow = r; }
-                }
-            }
+            for (int sl = 0; sl < 31; sl++) X[sl] = X[sl + 1];
+            X[31] = x0;
+        }
+        __syncthreads();
+        // ---- g[k][p_c] = X[p_k][c] -> shared memory in true order (slot sl holds working slot (ngroups + sl) mod 32) ----
+        if (rr_ < n) {
+            const int pr_ = sm.pinv[rr_];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-                const int orow = __shfl_xor_sync(0xffffffffu, brow, o);
-                if (ob > best || (ob == best && orow < brow)) { best = ob; brow = orow; }
-            }
-            const int p = brow;
-            const float2 xp = sm.colk[kb][p];
-            const float inv = 1.0f / best;
-            const float2 dd = make_float2(xp.x * inv, -xp.y * inv);
-            if (w == (p & 15)) {
-                const int ip = p >> 4;
-#pragma unroll
-                for (int jj = 0; jj < 4; jj++) {
-                    float2 v = X[0][jj];
-#pragma unroll
-                    for (int ii = 1; ii < 8; ii++) if (ii == ip) v = X[ii][jj];
-                    sm.prow[kb][l + 32 * jj] = c64mul(v, dd);
-                }
-            }
-            __syncthreads();
-            if (tid == 0) {          // after the barrier: no warp is still searching with used[]
-                if (!(best > 0.f) || !(best < 3.0e38f)) a.status[bl] = 1;
-                sm.used[p] = 1; sm.perm[k] = p; sm.pinv[p] = k;
-            }
-#pragma unroll
-            for (int ii = 0; ii < 8; ii++) {
-                const int r = w + 16 * ii;
-                const bool is_piv = (r == p);
-                const float2 xr = sm.colk[kb][r];                 // multiplier of the SCALED pivot row
-                const float2 f = c64mul(xr, dd);
-#pragma unroll
-                for (int jj = 0; jj < 4; jj++) {
-                    const int c = l + 32 * jj;
-                    const float2 pr = sm.prow[kb][c];
-                    float2 v = X[ii][jj];
-                    if (c == k) v = is_piv ? dd : make_float2(-f.x, -f.y);
-                    else if (is_piv) v = pr;
-                    else { v.x = fmaf(-xr.x, pr.x, v.x); v.x = fmaf(xr.y, pr.y, v.x); v.y = fmaf(-xr.x, pr.y, v.y); v.y = fmaf(-xr.y, pr.x, v.y); }
-                    X[ii][jj] = v;
+            for (int sl = 0; sl < 32; sl++) {
+                const int cw = 4 * ((ngroups + sl) & 31) + q;
+                if (cw < n) {
+                    int c = cw + shift; if (c >= n) c -= n;
+                    sm.g[pr_ * HC_LDG + sm.perm[c]] = X[sl];
                 }
             }
         }
         __syncthreads();
-        // ---- g[k][p_c] = X[p_k][c] -> shared memory in true order ----
-#pragma unroll
-        for (int ii = 0; ii < 8; ii++)
-#pragma unroll
-            for (int jj = 0; jj < 4; jj++) {
-                const int r = w + 16 * ii, c = l + 32 * jj;
-                if (r < n && c < n) sm.g[sm.pinv[r] * HC_LDG + sm.perm[c]] = X[ii][jj];
-            }
-        __syncthreads();
-        // ---- P_new = g (C P_prev), 32-column tiles ----
+        // ---- P_new = g (C P_prev), 64-column tiles: thread (w, l) takes rows w + 16 i, columns 2 l and 2 l + 1 of the tile ----
         const float2 *Pp = Pb[cur];
         float2 *Pn = Pb[cur ^ 1];
-        for (int j0 = 0; j0 < nc; j0 += 32) {
-            for (int idx = tid; idx < n * 32; idx += HC_NT) {
-                const int m = idx >> 5, jj = idx & 31, j = j0 + jj;
+        for (int j0 = 0; j0 < nc; j0 += HC_TW) {
+            for (int idx = tid; idx < n * HC_TW; idx += HC_NT) {
+                const int m = idx / HC_TW, jj = idx % HC_TW, j = j0 + jj;
                 float2 v = make_float2(0.f, 0.f);
                 if (j < nc) {
                     if (first) v = make_float2(m == j ? 1.f : 0.f, 0.f);
@@ -218,30 +241,35 @@ __global__ void __launch_bounds__(HC_NT, 1) half_sweep_c64_kernel(HC64Args a)
                     else {
                         const int ua = sm.ra[m], ub = sm.rb[m];
                         float sx = 0.f, sy = 0.f;
-                        if (ua >= 0) { const float2 q = Pp[ua * HC_NMAX + j]; sx += q.x; sy += q.y; }
-                        if (ub >= 0) { const float2 q = Pp[ub * HC_NMAX + j]; sx += q.x; sy += q.y; }
+                        if (ua >= 0) { const float2 qv = Pp[ua * HC_NMAX + j]; sx += qv.x; sy += qv.y; }
+                        if (ub >= 0) { const float2 qv = Pp[ub * HC_NMAX + j]; sx += qv.x; sy += qv.y; }
                         v = make_float2(sx, sy);
                     }
                 }
                 sm.Wt[m * HC_LDW + jj] = v;
             }
             __syncthreads();
-            float2 acc[8];
+            float2 acc[8][2];
 #pragma unroll
-            for (int ii = 0; ii < 8; ii++) acc[ii] = make_float2(0.f, 0.f);
+            for (int ii = 0; ii < 8; ii++) acc[ii][0] = acc[ii][1] = make_float2(0.f, 0.f);
             for (int m = 0; m < n; m++) {
-                const float2 wv = sm.Wt[m * HC_LDW + l];
+                const float4 wv = *reinterpret_cast<const float4 *>(&sm.Wt[m * HC_LDW + 2 * l]);
 #pragma unroll
                 for (int ii = 0; ii < 8; ii++) {
                     const float2 gv = sm.g[(w + 16 * ii) * HC_LDG + m];
-                    acc[ii].x = fmaf(gv.x, wv.x, acc[ii].x); acc[ii].x = fmaf(-gv.y, wv.y, acc[ii].x);
-                    acc[ii].y = fmaf(gv.x, wv.y, acc[ii].y); acc[ii].y = fmaf(gv.y, wv.x, acc[ii].y);
+                    acc[ii][0].x = fmaf(gv.x, wv.x, acc[ii][0].x); acc[ii][0].x = fmaf(-gv.y, wv.y, acc[ii][0].x);
+                    acc[ii][0].y = fmaf(gv.x, wv.y, acc[ii][0].y); acc[ii][0].y = fmaf(gv.y, wv.x, acc[ii][0].y);
+                    acc[ii][1].x = fmaf(gv.x, wv.z, acc[ii][1].x); acc[ii][1].x = fmaf(-gv.y, wv.w, acc[ii][1].x);
+                    acc[ii][1].y = fmaf(gv.x, wv.w, acc[ii][1].y); acc[ii][1].y = fmaf(gv.y, wv.z, acc[ii][1].y);
                 }
             }
 #pragma unroll
             for (int ii = 0; ii < 8; ii++) {
-                const int r = w + 16 * ii;
-                if (r < n && j0 + l < nc) Pn[r * HC_NMAX + j0 + l] = acc[ii];
+                const int r = w + 16 * ii, j = j0 + 2 * l;
+                if (r < n) {
+                    if (j < nc) Pn[r * HC_NMAX + j] = acc[ii][0];
+                    if (j + 1 < nc) Pn[r * HC_NMAX + j + 1] = acc[ii][1];
+                }
             }
             __syncthreads();
         }
