@@ -66,6 +66,9 @@ def parse():
     ap.add_argument("--form", default="half", choices=["half", "dense"], help="formulation of the sweep (include/rgf.h)")
     ap.add_argument("--no-guard", action="store_true", help="switch the near-neutrality guard off (rgf_set_guard 0)")
     ap.add_argument("--ldos", action="store_true", help="time the second workload instead (rgf_ldos, SURVEY.md 8(f) F-4): M, L as given, n-E energies")
+    ap.add_argument("--workload", default="", choices=["", "configs[3]-clean", "configs[3]", "configs[4]"],
+                    help="time another BASELINE.json config instead of the headline (one compact JSON line, no e2e / cpu legs)")
+    ap.add_argument("--precision", default="c128", choices=["c128", "c64"], help="with --workload: arithmetic of the sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -222,12 +225,56 @@ def run_ldos(a):
     rgf.rgf_destroy(plan)
 
 
+def run_other(a):
+    """The other BASELINE.json configs (not the headline line): one rgf_transmission call per step on the config's own
+    arrays (vacancies included), inputs resident in HBM, CUDA events around the timed steps."""
+    import torch
+    from paper_1107_5300_b200 import binding as rgf
+    w = {"configs[3]-clean": lambda: inputs.config3(disordered=False), "configs[3]": lambda: inputs.config3(disordered=True),
+         "configs[4]": inputs.config4}[a.workload]()
+    c64 = a.precision == "c64"
+    plan = rgf.rgf_plan_create(0, torch.cuda.current_stream().cuda_stream)
+    peak = rgf.rgf_fp64_peak_tflops(plan)
+    vac = None if w.vacancy is None else np.ascontiguousarray(w.vacancy[0])
+    rgf.rgf_set_device(plan, w.M, w.L, np.ascontiguousarray(w.onsite[0]), w.t, vac)
+    E = torch.from_numpy(w.energies).cuda()
+    T = torch.empty(w.n_E, dtype=torch.float64, device="cuda")
+    ok = (rgf.RGF_ESINGULAR,) if c64 else ()             # complex64 overflows in and next to the gap (DESIGN.md 5b): NaN + ESINGULAR
+    prec = rgf.RGF_C64 if c64 else rgf.RGF_C128
+    for _ in range(max(1, a.warmup)):
+        rgf.rgf_transmission(plan, E, w.n_E, w.eta, prec, T, ok)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(a.steps):
+        rgf.rgf_transmission(plan, E, w.n_E, w.eta, prec, T, ok)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / a.steps
+    st = rgf.rgf_get_stats(plan)
+    n = w.M // 2
+    flops = w.n_E * w.L * 2 * 16.0 * n ** 3               # executed: per half-step an (M/2) inverse + the (M/2)^3 propagator product
+    tf = flops / (ms * 1e-3) * 1e-12
+    fp32_peak = 148 * 128 * 2 * 1.965e-3                  # TFLOP/s, FFMA lanes x clock (DESIGN.md 5b)
+    print(json.dumps({"metric": METRIC, "value": w.n_E * w.L / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": a.steps, "warmup": a.warmup,
+                      "config": {"workload": w.name, "precision": a.precision, "formulation": "half"},
+                      "tflops_executed": tf, "roofline": {"bound": "alu" if c64 else "tensor", "achieved": tf, "peak": fp32_peak if c64 else peak,
+                                                          "unit": "TFLOP/s", "frac": tf / (fp32_peak if c64 else peak),
+                                                          "note": "whole call (all kernels), executed flops 2 x 16 (M/2)^3 per slice"},
+                      "phase_ms_last_step": {k: st[k] for k in ("ms_total", "ms_leads", "ms_sweep", "ms_trace", "ms_guard")},
+                      "guard_redone_energies": st["guard_redone"], "gpu_launches": st["launches"],
+                      "dtype": "f32" if c64 else "f64", "data": "synthetic"}))
+    rgf.rgf_destroy(plan)
+
+
 def main():
     a = parse()
     if a.impl == "reference":
         return run_reference(a)
     if a.ldos:
         return run_ldos(a)
+    if a.workload:
+        return run_other(a)
     import torch
     from paper_1107_5300_b200 import binding as rgf     # fails loudly if the CUDA library is missing
 
