@@ -370,6 +370,8 @@ def main():
             fl_inv, l_inv = update_flops_per_inverse(n_inv)
             flops_per_launch = fl_inv / max(l_inv, 1) * stats["cohort"]
             kernel_name = "gj32_update_kernel (FP64 DMMA.8x8x4)"
+            if n_inv > 256:      # generic path: its update launches are not event-timed (use --workload 'configs[4]' for the whole-call figure)
+                kernel_name = "gj_update_kernel<B> (n > 256: rank-B ping-pong update, not event-timed in this mode)"
             if a.form == "half":
                 flops_step = n_E * w.L * 2 * (8.0 * n_inv ** 3 + 8.0 * n_inv ** 3)     # executed: 2 x ((M/2) inverse + (M/2)^3 GEMM)
             else:
