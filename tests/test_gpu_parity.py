@@ -43,7 +43,7 @@ def tol(T):
 
 # ---- A4: the batched inverse on its own -----------------------------------------------------
 
-@pytest.mark.parametrize("n,batch", [(1, 3), (5, 4), (20, 7), (32, 2), (33, 3), (64, 2), (100, 5), (244, 6), (256, 2), (300, 2), (600, 1), (1100, 1), (2048, 1)])
+@pytest.mark.parametrize("n,batch", [(1, 3), (5, 4), (20, 7), (32, 2), (33, 3), (64, 2), (100, 5), (244, 6), (256, 2), (257, 2), (300, 2), (301, 3), (512, 2), (515, 1), (600, 1), (1100, 1), (1101, 1), (2048, 1)])
 def test_inverse_batched_matches_oracle_and_lapack(rgf, plan, oracle, n, batch):
     rng = np.random.default_rng(n * 31 + batch)
     A = rng.standard_normal((batch, n, n)) + 1j * rng.standard_normal((batch, n, n))
